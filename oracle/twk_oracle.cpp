@@ -1,0 +1,730 @@
+// twk_oracle.cpp -- TEST INFRASTRUCTURE ONLY.
+//
+// A plain, slow, obviously-correct CPU statement of what the hot path computes: finite-source binary-lens
+// magnification by contour integration, written from /root/reference/PAPER.md ("P:<line>" below) and the
+// readings listed in DESIGN.md.  It shares NO code with the CUDA path (own coefficient builder, own root
+// finder -- Durand-Kerner, not the product's Laguerre --, own linker, own integrator, own samplers).  Only
+// tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load it; the
+// product never does.
+//
+// Every routine is a template on the real type: `double` is the precision the method computes in (the
+// default face, the one timed as cpu_baseline), `long double` (x87 80-bit here) is the extended-precision
+// twin used to pin coefficient accuracy and classification.  prec = 0 -> double, 1 -> long double.
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"): coefficients vs mpmath elimination of Eq.(1); roots vs
+// Vieta/backward error; sum of residuals = 0; ghost 2-cycle geometry; 3-or-5 images, parity sum -1
+// (P:155-159); generalised point-source magnification sum = 1; z' and z'^z'' vs finite differences of tracked
+// images; single-lens limits (Paczynski point source, uniform-disk closed forms); large-rho limit;
+// mass-swap / reflection symmetries; brute-force ray shooting on tiny inputs; the Fig.1 / Fig.2 worked
+// examples.  Unpinned: adaptive-mode *sample positions* (only the value mu is compared).
+
+#include <algorithm>
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+template <class R> using Cx = std::complex<R>;
+
+template <class R> inline R wedge(const Cx<R>& a, const Cx<R>& b) { return a.real() * b.imag() - a.imag() * b.real(); }
+template <class R> inline R dot(const Cx<R>& a, const Cx<R>& b) { return a.real() * b.real() + a.imag() * b.imag(); }
+
+// ---------------------------------------------------------------------------------------------------------
+// O1. lens geometry, Eq.(2)
+// ---------------------------------------------------------------------------------------------------------
+template <class R> struct Lens {
+  R s, q, m1, m2, z1, z2;
+};
+template <class R> Lens<R> make_lens(double s_, double q_) {
+  Lens<R> L;
+  L.s = (R)s_;
+  L.q = (R)q_;
+  L.m1 = R(1) / (R(1) + L.q);
+  L.m2 = L.q / (R(1) + L.q);
+  L.z1 = -L.q * L.s / (R(1) + L.q);
+  L.z2 = L.s / (R(1) + L.q);
+  return L;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// O2. polynomial coefficients in the planet frame (planet at 0, primary at -s), Eq.(6), as printed.
+// ---------------------------------------------------------------------------------------------------------
+template <class R> void coeffs_eq6(const Cx<R>& y, R s, R m2, Cx<R> c[6]) {
+  const Cx<R> I(0, 1);
+  const Cx<R> yb = std::conj(y);
+  const Cx<R> vc = yb + s;            // v_c = ybar + s
+  const Cx<R> vp = R(1) + s * yb;     // v_p = 1 + s ybar
+  const R Iy = y.imag();
+  c[5] = -yb * vc;
+  c[4] = (yb * y - R(1) - R(2) * s * yb) * vc + m2 * s;
+  c[3] = (R(2) * y - s) * (vp * vc + R(2) * Iy * I - m2 * s) + R(4) * (m2 * s - y) * Iy * I;
+  c[2] = vp.real() * vp.real() * vc.real() + Iy * vp.real() * (R(1) - s * y).real() * I +
+         s * Iy * Iy * (R(2) + s * vc) + m2 * s * (R(2) * yb * (y - s) - (R(1) - s * y));
+  c[1] = m2 * s * ((s + R(2) * y) * vp + s * (R(2) * s * Iy * I - m2));
+  c[0] = s * s * m2 * m2 * y;
+}
+
+// The conventional form Eq.(4), with the OCR repair of c3 ("+ s [y + 2 ybar (ybar y - m2)]", DESIGN.md
+// reading E-1).  NOT on any path: kept only as the foil of the cancellation test.
+template <class R> void coeffs_eq4(const Cx<R>& y, R s, R m1, R m2, Cx<R> c[6]) {
+  const Cx<R> yb = std::conj(y);
+  c[5] = -yb * (yb + s);
+  c[4] = yb * (yb * (R(-2) * s + y) - R(1)) + s * (yb * (R(-2) * s + y) - m1);
+  c[3] = R(2) * yb * y - s * s * s * yb + s * s * (yb * (R(2) * y - yb) - m1) + s * (y + R(2) * yb * (yb * y - m2));
+  c[2] = y * (R(1) + s * s * s * yb) + s * (m1 + R(2) * y * yb * (R(1) + m2)) +
+         s * s * (yb * (m1 - m2) + y * (R(1) + m2 + yb * yb));
+  c[1] = m2 * s * (s * (m1 + y * (R(2) * yb + s)) + R(2) * y);
+  c[0] = s * s * m2 * m2 * y;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// O3. quintic roots: Durand-Kerner (Weierstrass) simultaneous iteration + Newton polish on the undeflated
+// polynomial.  Textbook; deliberately a different algorithm from the product's solver.
+// ---------------------------------------------------------------------------------------------------------
+template <class R> inline Cx<R> horner(const Cx<R> c[6], const Cx<R>& x) {
+  Cx<R> p = c[5];
+  for (int i = 4; i >= 0; --i) p = p * x + c[i];
+  return p;
+}
+template <class R> inline void horner2(const Cx<R> c[6], const Cx<R>& x, Cx<R>& p, Cx<R>& dp) {
+  p = c[5];
+  dp = Cx<R>(0, 0);
+  for (int i = 4; i >= 0; --i) {
+    dp = dp * x + p;
+    p = p * x + c[i];
+  }
+}
+
+template <class R> int quintic_roots_dk(const Cx<R> c[6], Cx<R> r[5]) {
+  const R eps = std::numeric_limits<R>::epsilon();
+  Cx<R> b[6];
+  for (int i = 0; i < 6; ++i) b[i] = c[i] / c[5];
+  // Fujiwara bound on the root moduli
+  R rad = 0;
+  for (int k = 1; k <= 5; ++k) {
+    R t = std::pow(std::abs(b[5 - k]) * (k == 5 ? R(0.5) : R(1)), R(1) / R(k));
+    rad = std::max(rad, t);
+  }
+  rad *= R(2);
+  if (!(rad > 0)) rad = 1;
+  const Cx<R> ctr = -b[4] / R(5);
+  const R r0 = R(0.5) * rad + std::abs(ctr) * R(0.1) + std::numeric_limits<R>::min();
+  const R twopi = R(2) * std::acos(R(-1));
+  for (int k = 0; k < 5; ++k) r[k] = ctr + std::polar(r0, twopi * R(k) / R(5) + R(0.4));
+  int sweep = 0, stalled = 0;
+  R best = std::numeric_limits<R>::infinity();
+  for (; sweep < 2000; ++sweep) {
+    R maxrel = 0;
+    for (int k = 0; k < 5; ++k) {
+      Cx<R> num = horner(b, r[k]);
+      Cx<R> den(1, 0);
+      for (int j = 0; j < 5; ++j)
+        if (j != k) den *= (r[k] - r[j]);
+      if (den == Cx<R>(0, 0)) den = Cx<R>(eps, eps);
+      Cx<R> d = num / den;
+      r[k] -= d;
+      maxrel = std::max(maxrel, std::abs(d) / std::max(std::abs(r[k]), std::numeric_limits<R>::min()));
+    }
+    if (maxrel < R(2) * eps) break;
+    // ill-conditioned clusters never reach 2 eps: stop once the update size has stopped shrinking
+    if (maxrel < R(0.5) * best) { best = maxrel; stalled = 0; } else if (maxrel < R(1e-6) && ++stalled >= 8) break;
+  }
+  // Newton polish on the full polynomial (3 steps; a step is taken only if it does not increase |P|)
+  for (int k = 0; k < 5; ++k) {
+    for (int it = 0; it < 3; ++it) {
+      Cx<R> p, dp;
+      horner2(c, r[k], p, dp);
+      if (dp == Cx<R>(0, 0)) break;
+      Cx<R> x1 = r[k] - p / dp;
+      if (std::abs(horner(c, x1)) <= std::abs(p)) r[k] = x1; else break;
+    }
+  }
+  return sweep;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// O1 + O4 + O5: one boundary point source -> five roots, residuals, Jacobians, classification, z', z'^z''.
+// ---------------------------------------------------------------------------------------------------------
+template <class R> struct Sample {
+  R theta;
+  Cx<R> zeta, dzeta;  // boundary point and d zeta / d theta = i rho e^{i theta}
+  Cx<R> c[6];         // Eq.(6) coefficients
+  Cx<R> z[5];         // all five roots, CM frame
+  Cx<R> Res[5];       // Eq.(12) residuals
+  R J[5];             // Eq.(7)
+  int kind[5];        // 0 ghost, +1 / -1 real image parity
+  Cx<R> zp[5];        // z' = dz/dtheta   (Eq.10, corrected: conj on f')
+  R w[5];             // z' ^ z''         (Eq.10, corrected: divided by J)
+  int nreal;
+  int repaired;       // parity repair fired (reading G-5)
+  int sweeps;
+};
+
+template <class R>
+void point_solve(const Lens<R>& L, const Cx<R>& zc, R rho, R theta, Sample<R>& S) {
+  S.theta = theta;
+  const Cx<R> e(std::cos(theta), std::sin(theta));
+  S.zeta = zc + rho * e;
+  S.dzeta = Cx<R>(0, 1) * rho * e;
+  const Cx<R> y = S.zeta - L.z2;
+  coeffs_eq6(y, L.s, L.m2, S.c);
+  Cx<R> eta[5];
+  S.sweeps = quintic_roots_dk(S.c, eta);
+  Cx<R> fpp[5], fp[5];
+  for (int k = 0; k < 5; ++k) {
+    // planet frame: z2 - z = -eta, z1 - z = -s - eta  (Eq.12 and Eq.7 are frame invariant)
+    const Cx<R> a = R(1) / (-L.s - eta[k]);
+    const Cx<R> b = R(1) / (-eta[k]);
+    const Cx<R> f = L.m1 * a + L.m2 * b;                           // Eq.(7)
+    fp[k] = L.m1 * a * a + L.m2 * b * b;                           // f'
+    fpp[k] = R(2) * (L.m1 * a * a * a + L.m2 * b * b * b);         // f''
+    S.Res[k] = y - eta[k] - std::conj(f);                          // Eq.(12)
+    S.J[k] = R(1) - std::norm(fp[k]);                              // Eq.(7)
+    S.z[k] = eta[k] + L.z2;
+  }
+  // residual detector, P:205-249, 2-cycle reading (G-1): the two largest-|R| roots a,b are a ghost
+  // pair iff R_a = z_b - z_a and R_b = z_a - z_b ("a pair of ghost images with opposite residuals").
+  int ia = 0, ib = 1;
+  {
+    int idx[5] = {0, 1, 2, 3, 4};
+    std::sort(idx, idx + 5, [&](int u, int v) { return std::abs(S.Res[u]) > std::abs(S.Res[v]); });
+    ia = idx[0];
+    ib = idx[1];
+  }
+  const Cx<R> dab = eta[ib] - eta[ia];
+  const bool ghost = std::abs(S.Res[ia] - dab) < std::abs(S.Res[ia]) && std::abs(S.Res[ib] + dab) < std::abs(S.Res[ib]);
+  S.nreal = 0;
+  int npos = 0;
+  for (int k = 0; k < 5; ++k) {
+    if (ghost && (k == ia || k == ib)) { S.kind[k] = 0; continue; }
+    S.kind[k] = (S.J[k] > 0) ? +1 : -1;   // Eq.(7)
+    S.nreal++;
+    npos += (S.kind[k] > 0);
+  }
+  // parity sum must be -1: (1+,2-) or (2+,3-).  If rounding next to the critical curve broke it, flip
+  // the smallest-|J| image of the over-represented parity (reading G-5).
+  S.repaired = 0;
+  const int want = (S.nreal - 1) / 2;
+  while (npos != want) {
+    int best = -1;
+    for (int k = 0; k < 5; ++k) {
+      if (S.kind[k] == 0) continue;
+      if ((npos > want) != (S.kind[k] > 0)) continue;
+      if (best < 0 || std::abs(S.J[k]) < std::abs(S.J[best])) best = k;
+    }
+    S.kind[best] = -S.kind[best];
+    npos += S.kind[best];   // +1 if flipped to +, -1 if flipped to -
+    S.repaired = 1;
+  }
+  for (int k = 0; k < 5; ++k) {
+    // Eq.(10) with the two OCR repairs (E-2, E-3)
+    S.zp[k] = (S.dzeta - std::conj(fp[k]) * std::conj(S.dzeta)) / S.J[k];
+    S.w[k] = (rho * rho + (S.zp[k] * S.zp[k] * S.dzeta * fpp[k]).imag()) / S.J[k];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// O6 + O7: one interval (theta_i -> theta_{i+1}): link, area piece, error piece.
+// ---------------------------------------------------------------------------------------------------------
+template <class R> struct Piece {
+  R dA, err;
+  int crossing;  // 0 none, +1 creation, -1 annihilation
+  int bad;       // leftover images are not exactly one (+,-) pair on one side
+  int nlinks;
+  int linkL[5], linkR[5];  // root indices of the linked pairs (diagnostics / tests)
+};
+
+template <class R>
+void eval_interval(const Sample<R>& A, const Sample<R>& B, R dth, Piece<R>& P) {
+  P.dA = 0;
+  P.err = 0;
+  P.crossing = 0;
+  P.bad = 0;
+  P.nlinks = 0;
+  int leftA[5], leftB[5], nLA = 0, nLB = 0;
+  for (int par = +1; par >= -1; par -= 2) {
+    int ia[5], ib[5], na = 0, nb = 0;
+    for (int k = 0; k < 5; ++k) {
+      if (A.kind[k] == par) ia[na++] = k;
+      if (B.kind[k] == par) ib[nb++] = k;
+    }
+    // injective maps of the smaller set into the larger one; keep the one of minimum total distance
+    const bool a_small = na <= nb;
+    const int* sm = a_small ? ia : ib;
+    const int* lg = a_small ? ib : ia;
+    const int ns = a_small ? na : nb, nl = a_small ? nb : na;
+    const Sample<R>& Ss = a_small ? A : B;
+    const Sample<R>& Sl = a_small ? B : A;
+    int perm[5] = {0, 1, 2, 3, 4}, bestp[5] = {0, 1, 2, 3, 4};
+    R best = std::numeric_limits<R>::infinity();
+    do {
+      R cost = 0;
+      for (int j = 0; j < ns; ++j) cost += std::abs(Ss.z[sm[j]] - Sl.z[lg[perm[j]]]);
+      if (cost < best) {
+        best = cost;
+        std::copy(perm, perm + 5, bestp);
+      }
+    } while (std::next_permutation(perm, perm + nl));
+    for (int j = 0; j < ns; ++j) {
+      const int ka = a_small ? sm[j] : lg[bestp[j]];
+      const int kb = a_small ? lg[bestp[j]] : sm[j];
+      P.linkL[P.nlinks] = ka;
+      P.linkR[P.nlinks] = kb;
+      P.nlinks++;
+      const Cx<R> dz = B.z[kb] - A.z[ka];
+      const R trap = R(0.5) * wedge(A.z[ka], dz);                                    // Eq.(9)
+      const R p1 = (A.w[ka] + B.w[kb]) * dth * dth * dth / R(24);                    // Eq.(10) dA^(p1)
+      const R p2 = wedge(dz, B.zp[kb] - A.zp[ka]) * dth / R(12);                     // Eq.(10) dA^(p2)
+      const R dAp = R(0.5) * (p1 + p2);
+      P.dA += R(par) * (trap + dAp);
+      const R E1 = std::abs(A.w[ka] - B.w[kb]) * dth * dth * dth / R(48);            // Eq.(17)
+      const R E2 = R(1.5) * std::abs(dAp * (std::norm(dz) / (dth * dth * std::abs(dot(A.zp[ka], B.zp[kb]))) - R(1)));
+      const R E3 = R(0.1) * std::abs(dAp) * dth * dth;
+      const R E4 = std::abs(p1 - p2);
+      P.err += E1 + E2 + E3 + E4;
+    }
+    for (int j = ns; j < nl; ++j) {
+      if (a_small) leftB[nLB++] = lg[bestp[j]]; else leftA[nLA++] = lg[bestp[j]];
+    }
+  }
+  if (nLA == 0 && nLB == 0) return;
+  // the extra real pair on the 5-image side connects to itself
+  const bool creation = (nLA == 0 && nLB == 2 && B.kind[leftB[0]] * B.kind[leftB[1]] == -1);
+  const bool annihil = (nLB == 0 && nLA == 2 && A.kind[leftA[0]] * A.kind[leftA[1]] == -1);
+  if (!creation && !annihil) {
+    P.bad = 1;
+    P.err = std::numeric_limits<R>::infinity();
+    return;
+  }
+  const Sample<R>& S = creation ? B : A;
+  const int* lf = creation ? leftB : leftA;
+  const int kp = (S.kind[lf[0]] > 0) ? lf[0] : lf[1];
+  const int km = (S.kind[lf[0]] > 0) ? lf[1] : lf[0];
+  const Cx<R> zpl = S.z[kp], zmi = S.z[km];
+  const Cx<R> d = zpl - zmi;
+  const R sq = std::sqrt(std::abs(dot(S.zp[kp], S.zp[km])));
+  const R dtt = std::abs(d) / sq;                                                    // Eq.(11) tilde Delta theta
+  const R corr = (S.w[kp] - S.w[km]) * dtt * dtt * dtt / R(24);                      // Eq.(11)
+  R dAp, chord, E2;
+  if (creation) {   // path z- -> z+   (reading S-2)
+    chord = R(0.5) * wedge(zmi, d);
+    dAp = -corr;
+    E2 = R(1.5) * std::abs(dot(d, S.zp[kp] - S.zp[km]) - R(2) * std::abs(d) * sq) * dtt;   // Eq.(18), E-5
+  } else {          // path z+ -> z-
+    chord = R(0.5) * wedge(zpl, -d);
+    dAp = +corr;
+    E2 = R(1.5) * std::abs(dot(d, S.zp[kp] - S.zp[km]) + R(2) * std::abs(d) * sq) * dtt;
+  }
+  P.crossing = creation ? +1 : -1;
+  P.dA += chord + dAp;
+  const R E1 = std::abs(S.w[kp] + S.w[km]) * dtt * dtt * dtt / R(48);                // Eq.(18)
+  const R E3 = R(0.1) * std::abs(dAp) * dth * dth;
+  P.err += E1 + E2 + E3;
+}
+
+const double kPi = 3.14159265358979323846264338327950288;
+template <class R> R pi_v() { return std::acos(R(-1)); }
+
+// ---------------------------------------------------------------------------------------------------------
+// Fixed-sampling face: theta_j = 2 pi j / N.
+// ---------------------------------------------------------------------------------------------------------
+template <class R>
+void images_fixed_one(double s, double q, double rho_, double zre, double zim, int N, double* out_z, int8_t* out_kind,
+                      int8_t* out_count, double* out_mu, double* out_err, int32_t* out_ncross, double* out_piece) {
+  const Lens<R> L = make_lens<R>(s, q);
+  const R rho = (R)rho_;
+  const Cx<R> zc((R)zre, (R)zim);
+  std::vector<Sample<R>> S(N);
+  const R twopi = R(2) * pi_v<R>();
+  for (int j = 0; j < N; ++j) {
+    point_solve(L, zc, rho, twopi * R(j) / R(N), S[j]);
+    for (int k = 0; k < 5; ++k) {
+      if (out_z) {
+        out_z[(size_t(j) * 5 + k) * 2 + 0] = (double)S[j].z[k].real();
+        out_z[(size_t(j) * 5 + k) * 2 + 1] = (double)S[j].z[k].imag();
+      }
+      if (out_kind) out_kind[size_t(j) * 5 + k] = (int8_t)S[j].kind[k];
+    }
+    if (out_count) out_count[j] = (int8_t)S[j].nreal;
+  }
+  R A = 0, E = 0;
+  int ncross = 0;
+  const R dth = twopi / R(N);
+  for (int j = 0; j < N; ++j) {
+    Piece<R> P;
+    eval_interval(S[j], S[(j + 1) % N], dth, P);
+    A += P.dA;
+    E += P.err;
+    ncross += (P.crossing != 0);
+    if (out_piece) {
+      out_piece[2 * j] = (double)P.dA;
+      out_piece[2 * j + 1] = (double)P.err;
+    }
+  }
+  if (out_mu) *out_mu = (double)(A / (pi_v<R>() * rho * rho));
+  if (out_err) *out_err = (double)(E / std::abs(A));
+  if (out_ncross) *out_ncross = ncross;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Adaptive face.  mode 0: the paper's sampler (readings A-1..A-6).
+//                 mode 1: the oracle's own converged reference (bisection of the worst intervals, O8).
+// ---------------------------------------------------------------------------------------------------------
+struct AdaptOpt {
+  int samples_per_iter, initial_samples, max_samples, subtract_avg_tol;
+};
+
+template <class R> struct Contour {
+  Lens<R> L;
+  Cx<R> zc;
+  R rho;
+  std::vector<Sample<R>> S;   // sorted by theta
+  std::vector<Piece<R>> P;    // P[i] = interval (S[i], S[i+1 mod n])
+  R twopi;
+  void init(int n0) {
+    S.resize(n0);
+    for (int j = 0; j < n0; ++j) point_solve(L, zc, rho, twopi * R(j) / R(n0), S[j]);
+    P.resize(n0);
+    for (int j = 0; j < n0; ++j) eval(j);
+  }
+  R dtheta(int i) const {
+    const int n = (int)S.size();
+    return (i + 1 < n) ? S[i + 1].theta - S[i].theta : twopi - S[i].theta + S[0].theta;
+  }
+  void eval(int i) {
+    const int n = (int)S.size();
+    eval_interval(S[i], S[(i + 1) % n], dtheta(i), P[i]);
+  }
+  // insert new angles (each strictly inside some interval), re-evaluate only the changed intervals
+  void insert(std::vector<R> th) {
+    std::sort(th.begin(), th.end());
+    std::vector<Sample<R>> S2;
+    std::vector<Piece<R>> P2;
+    std::vector<char> dirty;
+    const int n = (int)S.size();
+    size_t t = 0;
+    for (int i = 0; i < n; ++i) {
+      S2.push_back(S[i]);
+      P2.push_back(P[i]);
+      dirty.push_back(0);
+      const R hi = (i + 1 < n) ? S[i + 1].theta : twopi;
+      while (t < th.size() && th[t] < hi) {
+        if (th[t] > S2.back().theta) {
+          Sample<R> ns;
+          point_solve(L, zc, rho, th[t], ns);
+          dirty.back() = 1;
+          S2.push_back(ns);
+          P2.push_back(Piece<R>());
+          dirty.push_back(1);
+        }
+        ++t;
+      }
+    }
+    S.swap(S2);
+    P.swap(P2);
+    for (size_t i = 0; i < S.size(); ++i)
+      if (dirty[i]) eval((int)i);
+  }
+  void sums(R& A, R& E, int& nbad) const {
+    A = 0;
+    E = 0;
+    nbad = 0;
+    for (const auto& p : P) {
+      A += p.dA;
+      if (p.bad) nbad++; else E += p.err;
+    }
+  }
+};
+
+template <class R>
+void magnify_one(double s, double q, double rho_, double zre, double zim, double tol, int mode, const AdaptOpt& o,
+                 double* out_mu, double* out_err, int32_t* out_n, uint32_t* out_status, double* out_theta /*optional, max_samples*/) {
+  Contour<R> C;
+  C.L = make_lens<R>(s, q);
+  C.rho = (R)rho_;
+  C.zc = Cx<R>((R)zre, (R)zim);
+  C.twopi = R(2) * pi_v<R>();
+  const R rtol = (R)tol;
+  uint32_t status = 0;
+  if (!(s > 0) || !(q > 0) || !(rho_ > 0) || !std::isfinite(s) || !std::isfinite(q) || !std::isfinite(rho_) ||
+      !std::isfinite(zre) || !std::isfinite(zim)) {
+    if (out_mu) *out_mu = std::numeric_limits<double>::quiet_NaN();
+    if (out_err) *out_err = std::numeric_limits<double>::quiet_NaN();
+    if (out_n) *out_n = 0;
+    if (out_status) *out_status = 8;
+    return;
+  }
+  if (s < 0.1 || s > 10 || q < 1e-9) status |= 8;   // outside the validated domain, P:374 (flagged, still computed)
+  R A = 0, E = 0;
+  int nbad = 0;
+  if (mode == 0) {
+    const int K = o.samples_per_iter;
+    C.init(o.initial_samples);
+    for (;;) {
+      C.sums(A, E, nbad);
+      const int n = (int)C.S.size();
+      if (nbad == 0 && E <= rtol * std::abs(A)) { status |= 1; break; }           // P:272, A-1
+      if (n + K > o.max_samples) { status |= 2; break; }                          // P:326, A-6
+      // error-weighted inverse-transform sampling
+      std::vector<R> wgt(n);
+      const R avg = o.subtract_avg_tol ? rtol * std::abs(A) / R(n) : R(0);        // P:306, A-5
+      R W = 0;
+      for (int i = 0; i < n; ++i) {
+        wgt[i] = C.P[i].bad ? R(0) : std::max(C.P[i].err - avg, R(0));
+        W += wgt[i];
+      }
+      if (nbad) {   // inconsistent intervals take half of the quantiles (reading A-7)
+        const R wb = (W + rtol * std::abs(A)) / R(nbad);
+        W = 0;
+        for (int i = 0; i < n; ++i) {
+          if (C.P[i].bad) wgt[i] = wb;
+          W += wgt[i];
+        }
+      }
+      if (!(W > 0)) {
+        W = 0;
+        for (int i = 0; i < n; ++i) { wgt[i] = C.P[i].err; W += wgt[i]; }
+      }
+      std::vector<R> cum(n + 1);
+      cum[0] = 0;
+      for (int i = 0; i < n; ++i) cum[i + 1] = cum[i] + wgt[i];
+      std::vector<R> newth;
+      for (int k = 0; k < K; ++k) {
+        const R target = (R(k) + R(0.5)) / R(K) * cum[n];                         // quantiles, A-4
+        int i = int(std::upper_bound(cum.begin(), cum.end(), target) - cum.begin()) - 1;
+        i = std::min(std::max(i, 0), n - 1);
+        while (i < n - 1 && !(wgt[i] > 0)) ++i;
+        const R frac = wgt[i] > 0 ? (target - cum[i]) / wgt[i] : R(0.5);
+        const R th = C.S[i].theta + frac * C.dtheta(i);                           // linear interpolation
+        const R hi = (i + 1 < n) ? C.S[i + 1].theta : C.twopi;
+        if (th > C.S[i].theta && th < hi) newth.push_back(th);
+      }
+      if (newth.empty()) { status |= 2; break; }
+      C.insert(newth);
+    }
+  } else {
+    C.init(256);
+    for (;;) {
+      C.sums(A, E, nbad);
+      const int n = (int)C.S.size();
+      if (nbad == 0 && E <= R(0.1) * rtol * std::abs(A)) { status |= 1; break; }
+      if (n >= 65536) { status |= 2; break; }
+      std::vector<int> idx(n);
+      for (int i = 0; i < n; ++i) idx[i] = i;
+      const int m = (n + 7) / 8;
+      std::partial_sort(idx.begin(), idx.begin() + m, idx.end(), [&](int a, int b) {
+        const R ea = C.P[a].bad ? std::numeric_limits<R>::infinity() : C.P[a].err;
+        const R eb = C.P[b].bad ? std::numeric_limits<R>::infinity() : C.P[b].err;
+        return ea > eb;
+      });
+      std::vector<R> newth;
+      for (int k = 0; k < m; ++k) {
+        const int i = idx[k];
+        if (!C.P[i].bad && !(C.P[i].err > 0)) continue;
+        newth.push_back(C.S[i].theta + R(0.5) * C.dtheta(i));
+      }
+      if (newth.empty()) { status |= 2; break; }
+      C.insert(newth);
+    }
+  }
+  int rep = 0;
+  for (const auto& smp : C.S) rep |= smp.repaired;
+  if (rep || nbad) status |= 4;
+  if (out_mu) *out_mu = (double)(A / (pi_v<R>() * C.rho * C.rho));
+  if (out_err) *out_err = (double)(E / std::abs(A));
+  if (out_n) *out_n = (int32_t)C.S.size();
+  if (out_status) *out_status = status;
+  if (out_theta)
+    for (size_t i = 0; i < C.S.size() && (int)i < o.max_samples; ++i) out_theta[i] = (double)C.S[i].theta;
+}
+
+template <class R>
+void point_out(double s, double q, double rho, double zre, double zim, double theta, double* z, double* Res,
+                      double* J, int32_t* kind, double* zp, double* w, int32_t* info) {
+  Lens<R> L = make_lens<R>(s, q);
+  Sample<R> S;
+  point_solve(L, Cx<R>((R)zre, (R)zim), (R)rho, (R)theta, S);
+  for (int k = 0; k < 5; ++k) {
+    z[2 * k] = (double)S.z[k].real();  z[2 * k + 1] = (double)S.z[k].imag();
+    Res[2 * k] = (double)S.Res[k].real();  Res[2 * k + 1] = (double)S.Res[k].imag();
+    J[k] = (double)S.J[k];
+    kind[k] = S.kind[k];
+    zp[2 * k] = (double)S.zp[k].real();  zp[2 * k + 1] = (double)S.zp[k].imag();
+    w[k] = (double)S.w[k];
+  }
+  info[0] = S.nreal;
+  info[1] = S.repaired;
+  info[2] = S.sweeps;
+}
+
+}  // namespace
+
+// =========================================================================================================
+// C interface (ctypes).  All arrays are host arrays of double / int; complex = 2 consecutive doubles (re, im).
+// =========================================================================================================
+extern "C" {
+
+int orc_num_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+// Eq.(6) (form=6) or Eq.(4) (form=4) coefficients for source position zeta (CM frame).  out_c: 6 complex.
+void orc_coeffs(double s, double q, double zre, double zim, int form, int prec, double* out_c) {
+  if (prec) {
+    typedef long double R;
+    Lens<R> L = make_lens<R>(s, q);
+    Cx<R> c[6];
+    Cx<R> y = Cx<R>(zre, zim) - L.z2;
+    if (form == 6) coeffs_eq6(y, L.s, L.m2, c); else coeffs_eq4(y, L.s, L.m1, L.m2, c);
+    for (int i = 0; i < 6; ++i) { out_c[2 * i] = (double)c[i].real(); out_c[2 * i + 1] = (double)c[i].imag(); }
+  } else {
+    typedef double R;
+    Lens<R> L = make_lens<R>(s, q);
+    Cx<R> c[6];
+    Cx<R> y = Cx<R>(zre, zim) - L.z2;
+    if (form == 6) coeffs_eq6(y, L.s, L.m2, c); else coeffs_eq4(y, L.s, L.m1, L.m2, c);
+    for (int i = 0; i < 6; ++i) { out_c[2 * i] = c[i].real(); out_c[2 * i + 1] = c[i].imag(); }
+  }
+}
+
+// Roots of an arbitrary complex quintic (coefficients c0..c5) by the oracle's solver.
+void orc_quintic_roots(const double* c_in, int prec, double* out_roots) {
+  if (prec) {
+    typedef long double R;
+    Cx<R> c[6], r[5];
+    for (int i = 0; i < 6; ++i) c[i] = Cx<R>(c_in[2 * i], c_in[2 * i + 1]);
+    quintic_roots_dk(c, r);
+    for (int k = 0; k < 5; ++k) { out_roots[2 * k] = (double)r[k].real(); out_roots[2 * k + 1] = (double)r[k].imag(); }
+  } else {
+    typedef double R;
+    Cx<R> c[6], r[5];
+    for (int i = 0; i < 6; ++i) c[i] = Cx<R>(c_in[2 * i], c_in[2 * i + 1]);
+    quintic_roots_dk(c, r);
+    for (int k = 0; k < 5; ++k) { out_roots[2 * k] = r[k].real(); out_roots[2 * k + 1] = r[k].imag(); }
+  }
+}
+
+// One boundary point source: centre (zre, zim), radius rho, angle theta.
+void orc_point(double s, double q, double rho, double zre, double zim, double theta, int prec, double* z, double* Res,
+               double* J, int32_t* kind, double* zp, double* w, int32_t* info) {
+  if (prec) point_out<long double>(s, q, rho, zre, zim, theta, z, Res, J, kind, zp, w, info);
+  else point_out<double>(s, q, rho, zre, zim, theta, z, Res, J, kind, zp, w, info);
+}
+
+// Fixed-sampling face for a batch.  model_id may be NULL (then n_models is 1 or n_sources).
+// out_z [n][N][5][2], out_kind [n][N][5], out_count [n][N], out_mu [n], out_err [n], out_ncross [n],
+// out_piece [n][N][2] (dA, err per interval) -- every output pointer may be NULL.
+void orc_images_fixed(int64_t n_models, const double* s, const double* q, const double* rho, int64_t n_sources,
+                      const int32_t* model_id, const double* zeta, int N, int prec, int nthreads, double* out_z,
+                      int8_t* out_kind, int8_t* out_count, double* out_mu, double* out_err, int32_t* out_ncross,
+                      double* out_piece) {
+  (void)nthreads;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads > 0 ? nthreads : orc_num_threads())
+  for (int64_t i = 0; i < n_sources; ++i) {
+    const int64_t m = model_id ? model_id[i] : (n_models == 1 ? 0 : i);
+    double* oz = out_z ? out_z + size_t(i) * N * 10 : nullptr;
+    int8_t* ok = out_kind ? out_kind + size_t(i) * N * 5 : nullptr;
+    int8_t* oc = out_count ? out_count + size_t(i) * N : nullptr;
+    double* op = out_piece ? out_piece + size_t(i) * N * 2 : nullptr;
+    if (prec)
+      images_fixed_one<long double>(s[m], q[m], rho[m], zeta[2 * i], zeta[2 * i + 1], N, oz, ok, oc, out_mu ? out_mu + i : nullptr,
+                                    out_err ? out_err + i : nullptr, out_ncross ? out_ncross + i : nullptr, op);
+    else
+      images_fixed_one<double>(s[m], q[m], rho[m], zeta[2 * i], zeta[2 * i + 1], N, oz, ok, oc, out_mu ? out_mu + i : nullptr,
+                               out_err ? out_err + i : nullptr, out_ncross ? out_ncross + i : nullptr, op);
+  }
+}
+
+// Adaptive face for a batch.  mode 0 = the paper's sampler, mode 1 = the oracle's converged reference.
+void orc_magnify(int64_t n_models, const double* s, const double* q, const double* rho, int64_t n_sources,
+                 const int32_t* model_id, const double* zeta, double rel_tol, int mode, int samples_per_iter,
+                 int initial_samples, int max_samples, int subtract_avg_tol, int prec, int nthreads, double* out_mu,
+                 double* out_err, int32_t* out_nsamples, uint32_t* out_status) {
+  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol};
+  (void)nthreads;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads > 0 ? nthreads : orc_num_threads())
+  for (int64_t i = 0; i < n_sources; ++i) {
+    const int64_t m = model_id ? model_id[i] : (n_models == 1 ? 0 : i);
+    if (prec)
+      magnify_one<long double>(s[m], q[m], rho[m], zeta[2 * i], zeta[2 * i + 1], rel_tol, mode, o, out_mu ? out_mu + i : nullptr,
+                               out_err ? out_err + i : nullptr, out_nsamples ? out_nsamples + i : nullptr,
+                               out_status ? out_status + i : nullptr, nullptr);
+    else
+      magnify_one<double>(s[m], q[m], rho[m], zeta[2 * i], zeta[2 * i + 1], rel_tol, mode, o, out_mu ? out_mu + i : nullptr,
+                          out_err ? out_err + i : nullptr, out_nsamples ? out_nsamples + i : nullptr,
+                          out_status ? out_status + i : nullptr, nullptr);
+  }
+}
+
+// Sorted sample angles the paper-style sampler ends with, for one source (diagnostics).  Returns n.
+int orc_magnify_thetas(double s, double q, double rho, double zre, double zim, double rel_tol, int samples_per_iter,
+                       int initial_samples, int max_samples, int subtract_avg_tol, int prec, double* out_theta) {
+  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol};
+  int32_t n = 0;
+  if (prec) magnify_one<long double>(s, q, rho, zre, zim, rel_tol, 0, o, nullptr, nullptr, &n, nullptr, out_theta);
+  else magnify_one<double>(s, q, rho, zre, zim, rel_tol, 0, o, nullptr, nullptr, &n, nullptr, out_theta);
+  return n;
+}
+
+// O9. Brute-force inverse ray shooting: rays on a uniform grid of nx x ny cells over the image-plane
+// box [x0,x1] x [y0,y1]; a coarse cell is subdivided sub x sub when any of its corners or its centre lands
+// within (rho + margin) of the source centre.  Returns the magnification (hit area / (pi rho^2)).
+double orc_rayshoot(double s, double q, double rho, double zre, double zim, double x0, double x1, double y0, double y1,
+                    int nx, int ny, int sub, int nthreads) {
+  const Lens<double> L = make_lens<double>(s, q);
+  const double hx = (x1 - x0) / nx, hy = (y1 - y0) / ny;
+  auto map = [&](double x, double y, double& sx, double& sy) {
+    // Eq.(1): zeta = z + m1/(conj z1 - conj z) + m2/(conj z2 - conj z)
+    const double ax = x - L.z1, bx = x - L.z2;
+    const double da = ax * ax + y * y, db = bx * bx + y * y;
+    sx = x - L.m1 * ax / da - L.m2 * bx / db;
+    sy = y - L.m1 * y / da - L.m2 * y / db;
+  };
+  double total = 0;
+  (void)nthreads;
+#pragma omp parallel for schedule(dynamic, 8) reduction(+ : total) num_threads(nthreads > 0 ? nthreads : orc_num_threads())
+  for (int iy = 0; iy < ny; ++iy) {
+    double rowsum = 0;
+    for (int ix = 0; ix < nx; ++ix) {
+      const double cx = x0 + ix * hx, cy = y0 + iy * hy;
+      // distance of the mapped corners/centre from the source centre, and the local stretch of the map
+      double dmin = 1e300, dmax = 0;
+      double px[5] = {cx, cx + hx, cx, cx + hx, cx + 0.5 * hx}, py[5] = {cy, cy, cy + hy, cy + hy, cy + 0.5 * hy};
+      double sxs[5], sys[5];
+      for (int k = 0; k < 5; ++k) {
+        map(px[k], py[k], sxs[k], sys[k]);
+        const double d = std::hypot(sxs[k] - zre, sys[k] - zim);
+        dmin = std::min(dmin, d);
+        dmax = std::max(dmax, d);
+      }
+      double span = 0;
+      for (int k = 0; k < 4; ++k) span = std::max(span, std::hypot(sxs[k] - sxs[4], sys[k] - sys[4]));
+      if (!(dmin < rho + 2 * span) ) continue;           // whole cell maps outside the disk (with margin)
+      if (std::isfinite(dmax) && dmax < rho - 2 * span && span < 0.25 * rho) { rowsum += hx * hy; continue; }   // wholly inside
+      int hits = 0;
+      for (int jy = 0; jy < sub; ++jy)
+        for (int jx = 0; jx < sub; ++jx) {
+          double sx, sy;
+          map(cx + (jx + 0.5) * hx / sub, cy + (jy + 0.5) * hy / sub, sx, sy);
+          const double ddx = sx - zre, ddy = sy - zim;
+          hits += (ddx * ddx + ddy * ddy <= rho * rho);
+        }
+      rowsum += hx * hy * hits / double(sub * sub);
+    }
+    total += rowsum;
+  }
+  return total / (kPi * rho * rho);
+}
+
+}  // extern "C"
