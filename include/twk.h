@@ -1,0 +1,115 @@
+/* twk.h -- C ABI of the B200-native finite-source binary-lens magnification library (libtwk.so).
+ *
+ * The operation: for every source centre zeta_c in a batch, the magnification mu = (total area of all images of
+ * the uniform disk |zeta - zeta_c| <= rho under the binary-lens map, Eq.(1)) / (pi rho^2)
+ * (PAPER.md:35), computed by contour integration: sample the source boundary, build the
+ * quintic with the cancellation-free coefficients of Eq.(6), solve it in FP64, drop ghost roots
+ * with the residual detector, link images of adjacent samples incl. creation/annihilation at caustic
+ * crossings, sum the Stokes area with trapezium + parabolic corrections (Eq.(8)-(11)),
+ * estimate the error (Eq.(17)-(18)) and refine the boundary by error-weighted inverse-transform
+ * sampling until the estimate meets the requested relative accuracy.
+ *
+ * Conventions
+ *  - Coordinates: the paper's centre-of-mass frame, Einstein-radius units (Eq.(2)): primary at
+ *    z1 = -q s/(1+q), secondary at z2 = +s/(1+q), both on the real axis; q = m2/m1.
+ *  - "DEVICE" pointers are CUDA device pointers owned by the caller (e.g. torch tensors); the library never
+ *    frees, reallocates or retains them.  "HOST" pointers are ordinary host memory.
+ *  - complex arrays are interleaved (re, im) doubles.
+ *  - Device-pointer calls are asynchronous on `stream` and perform no host synchronisation.
+ *  - Return value: TWK_OK or a negative TWK_E* code from synchronous argument validation / CUDA runtime errors.
+ *    Device-side problems never abort a call: they set per-source status bits (TWK_ST_*).
+ *  - There is no CPU fallback: every entry point that computes needs a CUDA device.
+ */
+#ifndef TWK_H_
+#define TWK_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TWK_OK 0
+#define TWK_EINVAL (-1) /* null required pointer, N < 4, rel_tol <= 0, bad options, n_sources > max_sources */
+#define TWK_ENOMEM (-2) /* workspace allocation failed */
+#define TWK_ECUDA (-3)  /* a CUDA runtime call failed; twk_strerror gives the CUDA text of the last one */
+
+/* per-source status bits (out_status) */
+#define TWK_ST_CONVERGED 1u  /* error estimate <= rel_tol * |A|                                       */
+#define TWK_ST_CAP 2u        /* sample cap reached: value and estimated error returned as the paper does */
+#define TWK_ST_REPAIRED 4u   /* a sample's parity sum was not -1 and was repaired (reading G-5)        */
+#define TWK_ST_DOMAIN 8u     /* s, q outside the validated domain 0.1<=s<=10, q>=1e-9: still computed;   */
+                             /* non-finite / non-positive s, q, rho or non-finite zeta: out_mu = NaN             */
+#define TWK_ST_NUMERIC 16u   /* a non-finite value appeared in the solve (degenerate quintic, zeta on a lens)    */
+
+typedef struct twk_ctx twk_ctx; /* opaque; owns only its device scratch workspace */
+
+typedef struct {
+  int samples_per_iter; /* new boundary samples (= quantiles) per refinement iteration, default 64;  */
+                        /* must be 64 in this build (one thread per new sample, two warps per source)             */
+  int initial_samples;  /* uniform samples of the first iteration, default 64; must be 64 in this build    */
+  int max_samples;      /* sample cap per source, default 4096; 64 <= max_samples <= 4096                  */
+  int subtract_avg_tol; /* 1 = subtract the average tolerance from every interval error before sampling */
+} twk_options;
+
+/* Fill *opt with the defaults above. */
+void twk_default_options(twk_options* opt);
+
+/* Create a context able to process up to max_sources sources per call on the current CUDA device.
+ * opt == NULL means defaults.  Allocates the device workspace (twk_workspace_bytes) once; no allocation happens
+ * inside twk_magnify / twk_images_fixed.  *ctx is set to NULL on failure. */
+int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources);
+int twk_destroy(twk_ctx* ctx);
+
+/* Bytes of device workspace twk_create would allocate (host-side arithmetic only; needs no GPU). */
+size_t twk_workspace_bytes(const twk_options* opt, size_t max_sources);
+
+/* Adaptive mode (the hot path; BASELINE configs 2-5).
+ *   s, q, rho   DEVICE double[n_models]   lens separation, mass ratio, source radius per model
+ *   model_id    DEVICE int32[n_sources] or NULL; NULL means n_models == 1 (shared) or n_models == n_sources (identity)
+ *   zeta        DEVICE double[n_sources][2]  source centres (re, im)
+ *   rel_tol     requested relative accuracy of mu: stop when sum e_i <= rel_tol * |A|
+ *   out_mu      DEVICE double[n_sources]    required
+ *   out_err     DEVICE double[n_sources]    optional (NULL): estimated relative error sum e_i / |A|
+ *   out_nsamples DEVICE int32[n_sources]    optional: boundary samples used
+ *   out_status  DEVICE uint32[n_sources]    optional: TWK_ST_* bits
+ * n_sources == 0 is a no-op returning TWK_OK. */
+int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho, size_t n_sources,
+                const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu, double* out_err,
+                int32_t* out_nsamples, uint32_t* out_status, void* stream /* cudaStream_t */);
+
+/* Fixed-sampling mode (BASELINE config 1 and the parity harness): theta_j = 2 pi j / N, no adaptivity.
+ *   out_z       DEVICE double[n_sources][N][5][2]  optional: all five roots, CM frame, order unspecified
+ *   out_kind    DEVICE int8[n_sources][N][5]       optional: 0 ghost, +1 / -1 real image of that parity
+ *   out_count   DEVICE int8[n_sources][N]          optional: number of real images (3 or 5)
+ *   out_mu      DEVICE double[n_sources]           optional: fixed-N area sum / (pi rho^2)
+ *   out_err     DEVICE double[n_sources]           optional: fixed-N error estimate / |A|
+ * N >= 4. */
+int twk_images_fixed(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                     size_t n_sources, const int32_t* model_id, const double* zeta, int N, double* out_z,
+                     int8_t* out_kind, int8_t* out_count, double* out_mu, double* out_err, void* stream);
+
+/* End-to-end convenience with HOST buffers (same meaning as twk_magnify): copies the inputs host->device into the
+ * context's staging area, runs twk_magnify on `stream`, copies the outputs device->host and synchronises the
+ * stream before returning.  Optional outputs may be NULL. */
+int twk_magnify_host(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                     size_t n_sources, const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu,
+                     double* out_err, int32_t* out_nsamples, uint32_t* out_status, void* stream);
+
+/* Diagnostics of the last twk_magnify on this context (synchronises `stream`): number of sources handed to the
+ * refinement stages 2 and 3, and the number of kernels the call launched.  Any pointer may be NULL. */
+int twk_last_stats(twk_ctx* ctx, int64_t* n_stage2, int64_t* n_stage3, int* n_launches, void* stream);
+
+/* FP64 FMA throughput probe used for the ALU roofline denominator: runs `iters` dependent-chain DFMAs per thread
+ * (8 independent chains per thread, a full persistent grid) and returns the measured TFLOP/s (2 flop per DFMA) in
+ * *out_tflops.  Synchronous. */
+int twk_fp64_peak_probe(int iters, double* out_tflops);
+
+const char* twk_strerror(int code);
+const char* twk_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TWK_H_ */

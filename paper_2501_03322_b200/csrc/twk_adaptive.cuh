@@ -1,0 +1,244 @@
+// twk_adaptive.cuh -- a8 + a9: the adaptive contour loop for one source per 64-thread CTA (see twk_kernels.cuh).
+#pragma once
+
+#include "twk_kernels.cuh"
+
+namespace twk {
+
+struct AdaptArgs {
+  Batch b;
+  double tol;
+  int cap;               // sample capacity of this stage (<= 4096)
+  int subtract_avg_tol;
+  int final_stage;       // 1: cap reached -> return value + estimate with TWK_ST_CAP; 0: hand to next stage
+  const int32_t* list;   // worklist of source ids (null: all sources 0..n_sources-1)
+  const int* count;      // number of entries of `list` (device; null: n_sources)
+  int* cursor;           // dynamic work fetch counter (device, zeroed before launch)
+  uint8_t* pending;      // stage 1 only: pending[src] = 1 when the source needs stage 2
+  int32_t* next_list;    // stage 2 only: sources that need stage 3 ...
+  int* next_count;       // ... appended with atomicAdd
+  double* arena;         // stages 2/3: gridDim.x * cap records of kRecDoubles doubles
+  double* out_mu;
+  double* out_err;       // may be null
+  int32_t* out_nsamples; // may be null
+  uint32_t* out_status;  // may be null
+};
+
+__host__ __device__ inline size_t adaptive_smem_bytes(int cap, bool stage1) {
+  size_t doubles = 3 * (size_t)cap + 2 * kThreads + 8 + (stage1 ? kRecDoubles * kThreads : 0);
+  size_t ints = 2 * kThreads + 4;
+  return doubles * 8 + ints * 4 + (size_t)cap * 2;
+}
+
+template <bool kStage1>
+__global__ void __launch_bounds__(kThreads, kStage1 ? 6 : 4) adaptive_kernel(AdaptArgs p) {
+  extern __shared__ double sm[];
+  const int cap = p.cap;
+  double* theta = sm;            // [cap] sorted sample angles
+  double* dA = theta + cap;      // [cap] area piece of interval (i, i+1)
+  double* er = dA + cap;         // [cap] error piece of interval (i, i+1)
+  double* newth = er + cap;      // [64]  angle of quantile k
+  double* cth = newth + kThreads;   // [64] compacted new angles
+  double* scratch = cth + kThreads; // [8]
+  double* recs = scratch + 8;       // stage 1: [26][64] records
+  int* newint = reinterpret_cast<int*>(recs + (kStage1 ? kRecDoubles * kThreads : 0));   // [64] interval of quantile k
+  int* cint = newint + kThreads;    // [64] compacted
+  int* iscr = cint + kThreads;      // [4]
+  uint16_t* ids = reinterpret_cast<uint16_t*>(iscr + 4);   // [cap] arena id of the sample at each sorted position
+
+  const int t = threadIdx.x;
+  const int lane = t & 31, warp = t >> 5;
+  double* arena = kStage1 ? nullptr : p.arena + (size_t)blockIdx.x * (size_t)cap * kRecDoubles;
+  auto recref = [&](int id) -> RecRef {
+    return kStage1 ? RecRef{recs + id, kThreads} : RecRef{arena + (size_t)id * kRecDoubles, 1};
+  };
+  const long long total = p.count ? (long long)*p.count : p.b.n_sources;
+
+  for (;;) {
+    __syncthreads();
+    if (t == 0) iscr[0] = atomicAdd(p.cursor, 1);
+    __syncthreads();
+    const long long cur = iscr[0];
+    if (cur >= total) break;
+    const long long src = p.list ? (long long)p.list[cur] : cur;
+    const SourceParams S = load_source(p.b, src);
+    if (!S.valid) {
+      if (t == 0) {
+        p.out_mu[src] = nan("");
+        if (p.out_err) p.out_err[src] = nan("");
+        if (p.out_nsamples) p.out_nsamples[src] = 0;
+        if (p.out_status) p.out_status[src] = 8u;
+        if (kStage1) p.pending[src] = 0;
+      }
+      continue;
+    }
+    // ---- first iteration: 64 uniform samples theta_j = 2 pi j / 64 (reading A-3) ----------------------
+    int flags = 0;
+    {
+      const double th = kTwoPi * double(t) / double(kThreads);
+      flags |= point_solve(S.L, S.zc, S.rho, th, recref(t), nullptr, nullptr, nullptr);
+      theta[t] = th;
+      if (!kStage1) ids[t] = (uint16_t)t;
+    }
+    __syncthreads();
+    {
+      const Piece P = eval_interval(recref(t), recref((t + 1) & (kThreads - 1)), kTwoPi / double(kThreads));
+      dA[t] = P.dA;
+      er[t] = P.err;
+    }
+    int n = kThreads;
+    uint32_t status = S.status;
+    bool exhausted = false;
+    double A = 0.0, E = 0.0;
+    for (;;) {
+      __syncthreads();
+      // ---- area and error sums over all intervals (a7 reduction) ----------------------------------------------
+      double a = 0.0, e = 0.0;
+      for (int i = t; i < n; i += kThreads) {
+        a += dA[i];
+        e += er[i];
+      }
+      block_sum2(a, e, scratch);
+      A = a;
+      E = e;
+      const double tolA = p.tol * fabs(A);
+      if (!(isfinite(A) && isfinite(E))) { status |= 16u; break; }
+      if (E <= tolA) { status |= 1u; break; }                       // stop rule P:272, reading A-1
+      if (n + kThreads > cap) { exhausted = true; break; }          // cap P:326, reading A-6
+      if (kStage1) { exhausted = true; break; }                     // (cap == 64: unreachable, lets the compiler drop the rest)
+      // ---- a8: error-weighted inverse-transform sampling, 64 quantiles ---------------------------
+      const double avg = p.subtract_avg_tol ? tolA / double(n) : 0.0;   // "average tolerance", reading A-5
+      double W = 0.0, unused = 0.0;
+      for (int i = t; i < n; i += kThreads) W += fmax(er[i] - avg, 0.0);
+      block_sum2(W, unused, scratch);
+      const bool raw = !(W > 0.0);
+      if (raw) W = E;
+      const double scale = double(kThreads) / W;
+      newint[t] = -1;
+      double carry = 0.0;
+      for (int base = 0; base < n; base += kThreads) {
+        const int i = base + t;
+        const double w = (i < n) ? (raw ? er[i] : fmax(er[i] - avg, 0.0)) : 0.0;
+        double x = w;   // inclusive scan over the 64 threads
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const double y = __shfl_up_sync(0xffffffffu, x, o);
+          if (lane >= o) x += y;
+        }
+        __syncthreads();
+        if (lane == 31) scratch[4 + warp] = x;
+        __syncthreads();
+        const double w0 = scratch[4], w1 = scratch[5];
+        if (warp == 1) x += w0;
+        const double cum_incl = carry + x;
+        double cum_excl = __shfl_up_sync(0xffffffffu, cum_incl, 1);
+        if (lane == 0) cum_excl = (warp == 0) ? carry : carry + w0;   // bitwise the left neighbour's cum_incl
+        if (w > 0.0) {
+          // quantile k has target (k + 1/2)/64 * W (reading A-4); this interval owns those in [cum_excl, cum_incl)
+          const int klo = min(kThreads, max(0, (int)ceil(cum_excl * scale - 0.5)));
+          const int khi = min(kThreads, max(0, (int)ceil(cum_incl * scale - 0.5)));
+          const double th0 = theta[i];
+          const double hi = (i + 1 < n) ? theta[i + 1] : kTwoPi;
+          for (int k = klo; k < khi; ++k) {
+            const double target = (double(k) + 0.5) / double(kThreads) * W;
+            const double frac = (target - cum_excl) / w;
+            const double th = fma(frac, hi - th0, th0);              // linear interpolation
+            newth[k] = (th > th0 && th < hi) ? th : nan("");
+            newint[k] = i;
+          }
+        }
+        carry += w0 + w1;
+      }
+      __syncthreads();
+      // ---- drop invalid / duplicate angles, compact (ballot + prefix sum) --------------------------------------
+      bool v = (newint[t] >= 0) && (newth[t] == newth[t]);
+      if (v && t > 0 && newint[t - 1] == newint[t] && !(newth[t] > newth[t - 1])) v = false;
+      const unsigned bal = __ballot_sync(0xffffffffu, v);
+      if (lane == 0) iscr[1 + warp] = __popc(bal);
+      __syncthreads();
+      const int m = iscr[1] + iscr[2];
+      const int rank = __popc(bal & ((1u << lane) - 1u)) + (warp ? iscr[1] : 0);
+      if (v) {
+        cth[rank] = newth[t];
+        cint[rank] = newint[t];
+      }
+      __syncthreads();
+      if (m == 0) { exhausted = true; break; }
+      // ---- merge: old element j moves up by the number of new samples inserted before it ------------------------
+      for (int base = ((n - 1) / kThreads) * kThreads; base >= 0; base -= kThreads) {
+        const int j = base + t;
+        const bool have = j < n;
+        double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+        uint16_t v3 = 0;
+        int cnt = 0;
+        if (have) {
+          v0 = theta[j];
+          v1 = dA[j];
+          v2 = er[j];
+          v3 = ids[j];
+          int lo = 0, hiq = m;   // cnt = #{r : cint[r] < j}
+          while (lo < hiq) {
+            const int mid = (lo + hiq) >> 1;
+            if (cint[mid] < j) lo = mid + 1; else hiq = mid;
+          }
+          cnt = lo;
+        }
+        __syncthreads();
+        if (have) {
+          theta[j + cnt] = v0;
+          dA[j + cnt] = v1;
+          er[j + cnt] = v2;
+          ids[j + cnt] = v3;
+        }
+        __syncthreads();
+      }
+      // ---- solve the new samples (a1-a5 only for the newly added) -----------------------------------------
+      const int pos = (t < m) ? cint[t] + 1 + t : 0;
+      if (t < m) {
+        const double th = cth[t];
+        theta[pos] = th;
+        ids[pos] = (uint16_t)(n + t);
+        flags |= point_solve(S.L, S.zc, S.rho, th, recref(n + t), nullptr, nullptr, nullptr);
+      }
+      const int n_new = n + m;
+      __syncthreads();
+      // ---- re-evaluate only the intervals that changed ----------------------------------------------------
+      if (t < m) {
+        {
+          const Piece P = eval_interval(recref(ids[pos - 1]), recref(n + t), theta[pos] - theta[pos - 1]);
+          dA[pos - 1] = P.dA;
+          er[pos - 1] = P.err;
+        }
+        const bool last_in_group = (t == m - 1) || (cint[t + 1] != cint[t]);
+        if (last_in_group) {
+          const int nxt = (pos + 1 < n_new) ? pos + 1 : 0;
+          const double dth = (pos + 1 < n_new) ? theta[pos + 1] - theta[pos] : kTwoPi - theta[pos];
+          const Piece P = eval_interval(recref(n + t), recref(ids[nxt]), dth);
+          dA[pos] = P.dA;
+          er[pos] = P.err;
+        }
+      }
+      n = n_new;
+    }
+    // ---- outputs / hand-over ------------------------------------------------------------------------------------
+    const int rep = __syncthreads_or(flags & kPointRepaired);
+    const int nonf = __syncthreads_or(flags & kPointNonFinite);
+    if (t == 0) {
+      if (exhausted && !p.final_stage) {
+        if (kStage1) p.pending[src] = 1;
+        else p.next_list[atomicAdd(p.next_count, 1)] = (int32_t)src;
+      } else {
+        if (exhausted) status |= 2u;
+        if (rep) status |= 4u;
+        if (nonf) status |= 16u;
+        p.out_mu[src] = A / (kPi * S.rho * S.rho);
+        if (p.out_err) p.out_err[src] = E / fabs(A);
+        if (p.out_nsamples) p.out_nsamples[src] = n;
+        if (p.out_status) p.out_status[src] = status;
+        if (kStage1) p.pending[src] = 0;
+      }
+    }
+  }
+}
+
+}  // namespace twk

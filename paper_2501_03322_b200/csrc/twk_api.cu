@@ -1,0 +1,354 @@
+// twk_api.cu -- the C ABI of include/twk.h: argument validation, workspace, kernel launches.  No torch types.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/twk.h"
+#include "twk_adaptive.cuh"
+
+namespace {
+
+constexpr int kAssumedSMs = 148;        // B200; workspace sizing only (twk_workspace_bytes needs no GPU)
+constexpr int kStage2Cap = 512;         // sample capacity of refinement stage 2
+constexpr int kStage2CtasPerSM = 6;
+constexpr int kStage3CtasPerSM = 2;
+constexpr int kFixedTile = 128;
+
+thread_local char g_cuda_msg[256] = "";
+
+struct Plan {
+  int cap2, cap3;       // 0 = stage absent
+  int grid2, grid3;
+  size_t arena_doubles;
+};
+
+Plan make_plan(const twk_options& o, int sms) {
+  Plan P{};
+  const int maxs = o.max_samples;
+  P.cap2 = (maxs >= 2 * twk::kThreads) ? (maxs < kStage2Cap ? maxs : kStage2Cap) : 0;
+  P.cap3 = (maxs > kStage2Cap) ? maxs : 0;
+  P.grid2 = P.cap2 ? sms * kStage2CtasPerSM : 0;
+  P.grid3 = P.cap3 ? sms * kStage3CtasPerSM : 0;
+  const size_t a2 = (size_t)P.grid2 * P.cap2, a3 = (size_t)P.grid3 * P.cap3;
+  P.arena_doubles = (a2 > a3 ? a2 : a3) * twk::kRecDoubles;
+  return P;
+}
+
+size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
+
+struct Layout {
+  size_t counters, pending, list1, list2, arena, total;
+};
+Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
+  const Plan P = make_plan(o, sms);
+  Layout L{};
+  size_t off = 0;
+  L.counters = off; off += 256;
+  L.pending = off;  off += align256(max_sources);
+  L.list1 = off;    off += align256(max_sources * 4);
+  L.list2 = off;    off += align256(max_sources * 4);
+  L.arena = off;    off += align256(P.arena_doubles * 8);
+  L.total = off;
+  return L;
+}
+
+bool valid_options(const twk_options& o) {
+  return o.samples_per_iter == twk::kThreads && o.initial_samples == twk::kThreads && o.max_samples >= twk::kThreads &&
+         o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1);
+}
+
+int cuda_fail(cudaError_t e) {
+  snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: %s", cudaGetErrorString(e));
+  return TWK_ECUDA;
+}
+#define TWK_CUDA(x)                         \
+  do {                                      \
+    cudaError_t e_ = (x);                   \
+    if (e_ != cudaSuccess) return cuda_fail(e_); \
+  } while (0)
+
+}  // namespace
+
+struct twk_ctx {
+  twk_options opt;
+  size_t max_sources;
+  int sms;
+  Plan plan;
+  Layout lay;
+  char* ws;
+  // host staging for twk_magnify_host (allocated on first use)
+  char* stage;
+  size_t stage_bytes;
+  int last_launches;
+};
+
+extern "C" {
+
+void twk_default_options(twk_options* opt) {
+  if (!opt) return;
+  opt->samples_per_iter = 64;
+  opt->initial_samples = 64;
+  opt->max_samples = 4096;
+  opt->subtract_avg_tol = 1;
+}
+
+size_t twk_workspace_bytes(const twk_options* opt, size_t max_sources) {
+  twk_options o;
+  twk_default_options(&o);
+  if (opt) o = *opt;
+  if (!valid_options(o)) return 0;
+  return make_layout(o, max_sources, kAssumedSMs).total;
+}
+
+int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
+  if (!ctx) return TWK_EINVAL;
+  *ctx = nullptr;
+  twk_options o;
+  twk_default_options(&o);
+  if (opt) o = *opt;
+  if (!valid_options(o) || max_sources == 0 || max_sources > (size_t)0x7fffffff) return TWK_EINVAL;
+  int dev = 0, sms = 0;
+  TWK_CUDA(cudaGetDevice(&dev));
+  TWK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  twk_ctx* c = new (std::nothrow) twk_ctx();
+  if (!c) return TWK_ENOMEM;
+  c->opt = o;
+  c->max_sources = max_sources;
+  c->sms = sms;
+  c->plan = make_plan(o, sms);
+  c->lay = make_layout(o, max_sources, sms);
+  c->ws = nullptr;
+  c->stage = nullptr;
+  c->stage_bytes = 0;
+  c->last_launches = 0;
+  cudaError_t e = cudaMalloc((void**)&c->ws, c->lay.total);
+  if (e != cudaSuccess) {
+    delete c;
+    cudaGetLastError();
+    return e == cudaErrorMemoryAllocation ? TWK_ENOMEM : cuda_fail(e);
+  }
+  // opt in to the large dynamic shared memory of stage 3
+  const int cap_big = c->plan.cap3 ? c->plan.cap3 : (c->plan.cap2 ? c->plan.cap2 : twk::kThreads);
+  e = cudaFuncSetAttribute(twk::adaptive_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)twk::adaptive_smem_bytes(cap_big, false));
+  if (e != cudaSuccess) {
+    cudaFree(c->ws);
+    delete c;
+    return cuda_fail(e);
+  }
+  *ctx = c;
+  return TWK_OK;
+}
+
+int twk_destroy(twk_ctx* ctx) {
+  if (!ctx) return TWK_OK;
+  if (ctx->ws) cudaFree(ctx->ws);
+  if (ctx->stage) cudaFree(ctx->stage);
+  delete ctx;
+  return TWK_OK;
+}
+
+static int check_batch(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                       size_t n_sources, const int32_t* model_id, const double* zeta) {
+  if (!ctx) return TWK_EINVAL;
+  if (n_sources == 0) return TWK_OK;
+  if (!s || !q || !rho || !zeta || n_models == 0) return TWK_EINVAL;
+  if (n_sources > ctx->max_sources) return TWK_EINVAL;
+  if (!model_id && n_models != 1 && n_models != n_sources) return TWK_EINVAL;
+  return TWK_OK;
+}
+
+int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho, size_t n_sources,
+                const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu, double* out_err,
+                int32_t* out_nsamples, uint32_t* out_status, void* stream_) {
+  const int rc = check_batch(ctx, n_models, s, q, rho, n_sources, model_id, zeta);
+  if (rc != TWK_OK) return rc;
+  if (n_sources == 0) return TWK_OK;
+  if (!out_mu || !(rel_tol > 0.0)) return TWK_EINVAL;
+  cudaStream_t stream = (cudaStream_t)stream_;
+  const Plan& P = ctx->plan;
+  int* counters = reinterpret_cast<int*>(ctx->ws + ctx->lay.counters);
+  // counters: [0] cursor1, [1] count1 (stage-2 worklist), [2] cursor2, [3] count2 (stage-3 worklist), [4] cursor3
+  TWK_CUDA(cudaMemsetAsync(counters, 0, 64, stream));
+  twk::AdaptArgs a{};
+  a.b = twk::Batch{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources};
+  a.tol = rel_tol;
+  a.subtract_avg_tol = ctx->opt.subtract_avg_tol;
+  a.out_mu = out_mu;
+  a.out_err = out_err;
+  a.out_nsamples = out_nsamples;
+  a.out_status = out_status;
+  a.arena = reinterpret_cast<double*>(ctx->ws + ctx->lay.arena);
+  a.pending = reinterpret_cast<uint8_t*>(ctx->ws + ctx->lay.pending);
+  int32_t* list1 = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list1);
+  int32_t* list2 = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list2);
+  int launches = 0;
+  // ---- stage 1: every source, 64 samples, records in shared memory ------------------------------------------------
+  {
+    twk::AdaptArgs a1 = a;
+    a1.cap = twk::kThreads;
+    a1.final_stage = P.cap2 ? 0 : 1;
+    a1.list = nullptr;
+    a1.count = nullptr;
+    a1.cursor = counters + 0;
+    const long long resident = (long long)ctx->sms * 6;
+    const int grid = (int)((long long)n_sources < resident ? (long long)n_sources : resident);
+    twk::adaptive_kernel<true><<<grid, twk::kThreads, twk::adaptive_smem_bytes(twk::kThreads, true), stream>>>(a1);
+    ++launches;
+  }
+  if (P.cap2) {
+    // ---- a9: compact the unfinished sources (ballot + prefix sum) ---------------------------------------------------
+    const long long blocks = ((long long)n_sources + 255) / 256;
+    const int grid = (int)(blocks < 4096 ? blocks : 4096);
+    twk::compact_kernel<<<grid, 256, 0, stream>>>(a.pending, (long long)n_sources, list1, counters + 1);
+    ++launches;
+    // ---- stage 2 -----------------------------------------------------------------------------------------------------
+    twk::AdaptArgs a2 = a;
+    a2.cap = P.cap2;
+    a2.final_stage = P.cap3 ? 0 : 1;
+    a2.list = list1;
+    a2.count = counters + 1;
+    a2.cursor = counters + 2;
+    a2.next_list = list2;
+    a2.next_count = counters + 3;
+    twk::adaptive_kernel<false><<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2, false), stream>>>(a2);
+    ++launches;
+  }
+  if (P.cap3) {
+    twk::AdaptArgs a3 = a;
+    a3.cap = P.cap3;
+    a3.final_stage = 1;
+    a3.list = list2;
+    a3.count = counters + 3;
+    a3.cursor = counters + 4;
+    twk::adaptive_kernel<false><<<P.grid3, twk::kThreads, twk::adaptive_smem_bytes(P.cap3, false), stream>>>(a3);
+    ++launches;
+  }
+  ctx->last_launches = launches;
+  TWK_CUDA(cudaGetLastError());
+  return TWK_OK;
+}
+
+int twk_images_fixed(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                     size_t n_sources, const int32_t* model_id, const double* zeta, int N, double* out_z,
+                     int8_t* out_kind, int8_t* out_count, double* out_mu, double* out_err, void* stream_) {
+  const int rc = check_batch(ctx, n_models, s, q, rho, n_sources, model_id, zeta);
+  if (rc != TWK_OK) return rc;
+  if (n_sources == 0) return TWK_OK;
+  if (N < 4) return TWK_EINVAL;
+  cudaStream_t stream = (cudaStream_t)stream_;
+  twk::Batch b{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources};
+  const size_t smem = (size_t)(twk::kRecDoubles * kFixedTile + 2 * twk::kRecDoubles + 2 * (kFixedTile / 32)) * 8;
+  const long long resident = (long long)ctx->sms * 8;
+  const int grid = (int)((long long)n_sources < resident ? (long long)n_sources : resident);
+  twk::fixed_kernel<kFixedTile><<<grid, kFixedTile, smem, stream>>>(b, N, out_z, out_kind, out_count, out_mu, out_err);
+  ctx->last_launches = 1;
+  TWK_CUDA(cudaGetLastError());
+  return TWK_OK;
+}
+
+int twk_magnify_host(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                     size_t n_sources, const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu,
+                     double* out_err, int32_t* out_nsamples, uint32_t* out_status, void* stream_) {
+  const int rc = check_batch(ctx, n_models, s, q, rho, n_sources, model_id, zeta);
+  if (rc != TWK_OK) return rc;
+  if (n_sources == 0) return TWK_OK;
+  if (!out_mu || !(rel_tol > 0.0)) return TWK_EINVAL;
+  cudaStream_t stream = (cudaStream_t)stream_;
+  // staging layout (device): s, q, rho [n_models each] | model_id | zeta | mu | err | nsamples | status
+  const size_t need = align256(n_models * 8) * 3 + align256(n_sources * 4) + align256(n_sources * 16) +
+                      align256(n_sources * 8) * 2 + align256(n_sources * 4) * 2;
+  if (need > ctx->stage_bytes) {
+    if (ctx->stage) cudaFree(ctx->stage);
+    ctx->stage = nullptr;
+    ctx->stage_bytes = 0;
+    cudaError_t e = cudaMalloc((void**)&ctx->stage, need);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      return e == cudaErrorMemoryAllocation ? TWK_ENOMEM : cuda_fail(e);
+    }
+    ctx->stage_bytes = need;
+  }
+  char* p = ctx->stage;
+  double* d_s = (double*)p;      p += align256(n_models * 8);
+  double* d_q = (double*)p;      p += align256(n_models * 8);
+  double* d_rho = (double*)p;    p += align256(n_models * 8);
+  int32_t* d_mid = (int32_t*)p;  p += align256(n_sources * 4);
+  double* d_zeta = (double*)p;   p += align256(n_sources * 16);
+  double* d_mu = (double*)p;     p += align256(n_sources * 8);
+  double* d_err = (double*)p;    p += align256(n_sources * 8);
+  int32_t* d_ns = (int32_t*)p;   p += align256(n_sources * 4);
+  uint32_t* d_st = (uint32_t*)p;
+  TWK_CUDA(cudaMemcpyAsync(d_s, s, n_models * 8, cudaMemcpyHostToDevice, stream));
+  TWK_CUDA(cudaMemcpyAsync(d_q, q, n_models * 8, cudaMemcpyHostToDevice, stream));
+  TWK_CUDA(cudaMemcpyAsync(d_rho, rho, n_models * 8, cudaMemcpyHostToDevice, stream));
+  if (model_id) TWK_CUDA(cudaMemcpyAsync(d_mid, model_id, n_sources * 4, cudaMemcpyHostToDevice, stream));
+  TWK_CUDA(cudaMemcpyAsync(d_zeta, zeta, n_sources * 16, cudaMemcpyHostToDevice, stream));
+  const int r2 = twk_magnify(ctx, n_models, d_s, d_q, d_rho, n_sources, model_id ? d_mid : nullptr, d_zeta, rel_tol, d_mu,
+                             out_err ? d_err : nullptr, out_nsamples ? d_ns : nullptr, out_status ? d_st : nullptr, stream_);
+  if (r2 != TWK_OK) return r2;
+  TWK_CUDA(cudaMemcpyAsync(out_mu, d_mu, n_sources * 8, cudaMemcpyDeviceToHost, stream));
+  if (out_err) TWK_CUDA(cudaMemcpyAsync(out_err, d_err, n_sources * 8, cudaMemcpyDeviceToHost, stream));
+  if (out_nsamples) TWK_CUDA(cudaMemcpyAsync(out_nsamples, d_ns, n_sources * 4, cudaMemcpyDeviceToHost, stream));
+  if (out_status) TWK_CUDA(cudaMemcpyAsync(out_status, d_st, n_sources * 4, cudaMemcpyDeviceToHost, stream));
+  TWK_CUDA(cudaStreamSynchronize(stream));
+  return TWK_OK;
+}
+
+int twk_last_stats(twk_ctx* ctx, int64_t* n_stage2, int64_t* n_stage3, int* n_launches, void* stream_) {
+  if (!ctx) return TWK_EINVAL;
+  int h[8] = {0};
+  TWK_CUDA(cudaMemcpyAsync(h, ctx->ws + ctx->lay.counters, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream_));
+  TWK_CUDA(cudaStreamSynchronize((cudaStream_t)stream_));
+  if (n_stage2) *n_stage2 = h[1];
+  if (n_stage3) *n_stage3 = h[3];
+  if (n_launches) *n_launches = ctx->last_launches;
+  return TWK_OK;
+}
+
+int twk_fp64_peak_probe(int iters, double* out_tflops) {
+  if (iters <= 0 || !out_tflops) return TWK_EINVAL;
+  int dev = 0, sms = 0;
+  TWK_CUDA(cudaGetDevice(&dev));
+  TWK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  double* d = nullptr;
+  TWK_CUDA(cudaMalloc((void**)&d, 8));
+  cudaEvent_t e0, e1;
+  TWK_CUDA(cudaEventCreate(&e0));
+  TWK_CUDA(cudaEventCreate(&e1));
+  const int grid = sms * 8, block = 256;
+  twk::dfma_probe_kernel<<<grid, block>>>(iters / 8 + 1, d);   // warm-up
+  float best = 1e30f;
+  for (int rep = 0; rep < 3; ++rep) {
+    TWK_CUDA(cudaEventRecord(e0));
+    twk::dfma_probe_kernel<<<grid, block>>>(iters, d);
+    TWK_CUDA(cudaEventRecord(e1));
+    TWK_CUDA(cudaEventSynchronize(e1));
+    float ms = 0;
+    TWK_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    if (ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d);
+  TWK_CUDA(cudaGetLastError());
+  const double flop = 2.0 * 8.0 * (double)iters * (double)grid * (double)block;
+  *out_tflops = flop / ((double)best * 1e-3) / 1e12;
+  return TWK_OK;
+}
+
+const char* twk_strerror(int code) {
+  switch (code) {
+    case TWK_OK: return "ok";
+    case TWK_EINVAL: return "invalid argument";
+    case TWK_ENOMEM: return "out of device memory for the workspace";
+    case TWK_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA runtime error";
+    default: return "unknown twk error code";
+  }
+}
+
+const char* twk_version(void) { return "twk 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,269 @@
+// twk_contour.cuh -- per-sample record (a1, a4, a5) and per-interval link + area + error (a6, a7).
+// See twk_device.cuh for the citation key.
+#pragma once
+
+#include "twk_device.cuh"
+
+namespace twk {
+
+// ------------------------------------------------------------------------------------------------------------
+// Sample record: what an interval needs from one boundary sample.  26 doubles, element e at base[e * stride]:
+//   [0..4]  Re z      slots 0,1 = positive-parity images, slots 2,3,4 = negative-parity images
+//   [5..9]  Im z      (slot 1 and slot 4 are filled only when the sample has 5 real images)
+//   [10..14] Re z'    z' = dz/dtheta, Eq.(10) (conj on f' restored)
+//   [15..19] Im z'
+//   [20..24] z'^z''   Eq.(10) (division by J restored)
+//   [25]    nreal (3 or 5) + 8 * repaired, stored as a double
+// In shared memory the record is a column of a [26][TILE] array (stride = TILE, conflict-free); in the global
+// arena it is 26 contiguous doubles (stride = 1, 208 B).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kRecDoubles = 26;
+constexpr int kZX = 0, kZY = 5, kPX = 10, kPY = 15, kW = 20, kNR = 25;
+
+struct RecRef {
+  double* base;
+  int stride;
+  TWK_HD double& at(int e) const { return base[e * stride]; }
+  TWK_HD cd z(int slot) const { return mk(base[(kZX + slot) * stride], base[(kZY + slot) * stride]); }
+  TWK_HD cd zp(int slot) const { return mk(base[(kPX + slot) * stride], base[(kPY + slot) * stride]); }
+  TWK_HD double w(int slot) const { return base[(kW + slot) * stride]; }
+  TWK_HD int nreal() const { return int(base[kNR * stride]) & 7; }
+  TWK_HD int repaired() const { return int(base[kNR * stride]) >> 3; }
+};
+
+constexpr int kPointRepaired = 1;   // parity sum was not -1 and was repaired (G-5)
+constexpr int kPointNonFinite = 2;  // a root or a derived quantity is not finite
+
+// ------------------------------------------------------------------------------------------------------------
+// a1 + a2 + a3 + a4 + a5: one boundary point source.
+// Writes the record; optionally the five roots (CM frame), their kinds and the real-image count.
+// ------------------------------------------------------------------------------------------------------------
+TWK_HD int point_solve(const Lens& L, cd zc, double rho, double theta, RecRef rec, double* out_z, int8_t* out_kind,
+                       int8_t* out_count) {
+  double sn, cs;
+  sincos(theta, &sn, &cs);
+  const cd zeta = mk(fma(rho, cs, zc.x), fma(rho, sn, zc.y));
+  const cd dzeta = mk(-rho * sn, rho * cs);                     // zeta' = i rho e^{i theta}
+  const cd y = mk(zeta.x - L.z2, zeta.y);
+  cd c[6], eta[5];
+  coeffs_eq6(y, L.s, L.m2, c);
+  quintic_roots(c, eta);
+
+  // a4: f', f'', residual, Jacobian in the planet frame (z2 - z = -eta, z1 - z = -s - eta; both are frame
+  // invariant)
+  cd fp[5], fpp[5], Res[5];
+  double J[5], R2[5];
+  bool finite = true;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const cd a = crecip(mk(-L.s - eta[k].x, -eta[k].y));
+    const cd b = crecip(-eta[k]);
+    const cd a2 = a * a, b2 = b * b;
+    const cd f = L.m1 * a + L.m2 * b;                    // Eq.(7)
+    fp[k] = L.m1 * a2 + L.m2 * b2;
+    fpp[k] = 2.0 * (L.m1 * (a2 * a) + L.m2 * (b2 * b));
+    Res[k] = mk(y.x - eta[k].x - f.x, y.y - eta[k].y + f.y);   // Eq.(12): y - eta - conj(f)
+    J[k] = 1.0 - norm2(fp[k]);                           // Eq.(7)
+    R2[k] = norm2(Res[k]);
+    finite = finite && isfinite(R2[k]) && isfinite(J[k]);
+  }
+  // a5: residual detector, 2-cycle reading (G-1): the two largest-|R| roots (ia, ib) are a ghost pair iff
+  // R_ia = eta_ib - eta_ia and R_ib = eta_ia - eta_ib ("a pair of ghost images with opposite residuals").
+  int ia = 0;
+#pragma unroll
+  for (int k = 1; k < 5; ++k)
+    if (R2[k] > R2[ia]) ia = k;
+  int ib = (ia == 0) ? 1 : 0;
+#pragma unroll
+  for (int k = 0; k < 5; ++k)
+    if (k != ia && R2[k] > R2[ib]) ib = k;
+  cd eA = eta[0], eB = eta[0], rA = Res[0], rB = Res[0];
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    if (k == ia) { eA = eta[k]; rA = Res[k]; }
+    if (k == ib) { eB = eta[k]; rB = Res[k]; }
+  }
+  const cd dab = eB - eA;
+  const bool ghost = norm2(rA - dab) < norm2(rA) && norm2(rB + dab) < norm2(rB);
+  int kind[5];
+  int nreal = 0, npos = 0;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const bool g = ghost && (k == ia || k == ib);
+    kind[k] = g ? 0 : (J[k] > 0.0 ? 1 : -1);             // Eq.(7)
+    nreal += !g;
+    npos += (kind[k] > 0);
+  }
+  // parity sum must be -1.  Repair by flipping the smallest-|J| image of the over-represented parity.
+  int flags = finite ? 0 : kPointNonFinite;
+  const int want = (nreal - 1) >> 1;
+  for (int guard = 0; guard < 5 && npos != want; ++guard) {
+    const int over = (npos > want) ? 1 : -1;
+    int best = -1;
+    double bj = 1e300;
+#pragma unroll
+    for (int k = 0; k < 5; ++k)
+      if (kind[k] == over && fabs(J[k]) < bj) { bj = fabs(J[k]); best = k; }
+#pragma unroll
+    for (int k = 0; k < 5; ++k)
+      if (k == best) kind[k] = -over;
+    npos -= over;
+    flags |= kPointRepaired;
+  }
+  // record: positives to slots 0.., negatives to slots 2..
+  int sp = 0, sm = 2;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const cd z = mk(eta[k].x + L.z2, eta[k].y);
+    if (out_z) { out_z[2 * k] = z.x; out_z[2 * k + 1] = z.y; }
+    if (out_kind) out_kind[k] = (int8_t)kind[k];
+    if (kind[k] != 0) {
+      const int slot = (kind[k] > 0) ? sp++ : sm++;
+      const double invJ = 1.0 / J[k];
+      // z' = (zeta' - conj(f') conj(zeta')) / J                       Eq.(10), repaired (E-2)
+      const cd t = conj(fp[k]) * conj(dzeta);
+      const cd zp = mk((dzeta.x - t.x) * invJ, (dzeta.y - t.y) * invJ);
+      // z'^z'' = (rho^2 + Im[z'^2 zeta' f'']) / J                     Eq.(10), repaired (E-3)
+      const cd u = (zp * zp) * (dzeta * fpp[k]);
+      const double w = fma(rho, rho, u.y) * invJ;
+      rec.at(kZX + slot) = z.x;
+      rec.at(kZY + slot) = z.y;
+      rec.at(kPX + slot) = zp.x;
+      rec.at(kPY + slot) = zp.y;
+      rec.at(kW + slot) = w;
+    }
+  }
+  rec.at(kNR) = double(nreal + ((flags & kPointRepaired) ? 8 : 0));
+  if (out_count) *out_count = (int8_t)nreal;
+  return flags;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a6 + a7: one interval theta_A -> theta_B (dth = theta_B - theta_A > 0).
+// ------------------------------------------------------------------------------------------------------------
+struct Piece {
+  double dA, err;
+  int crossing;   // 0 none, +1 creation, -1 annihilation
+};
+
+TWK_HD void link_terms(const RecRef& A, const RecRef& B, int ka, int kb, double par, double dth, double& dA,
+                       double& err) {
+  const cd zA = A.z(ka), zB = B.z(kb), pA = A.zp(ka), pB = B.zp(kb);
+  const double wA = A.w(ka), wB = B.w(kb);
+  const cd dz = zB - zA;
+  const double dth2 = dth * dth, dth3 = dth2 * dth;
+  const double trap = 0.5 * wedge(zA, dz);                              // Eq.(9)
+  const double p1 = (wA + wB) * dth3 * (1.0 / 24.0);                    // Eq.(10) dA^(p1)
+  const double p2 = wedge(dz, pB - pA) * dth * (1.0 / 12.0);            // Eq.(10) dA^(p2)
+  const double dAp = 0.5 * (p1 + p2);
+  dA += par * (trap + dAp);
+  const double E1 = fabs(wA - wB) * dth3 * (1.0 / 48.0);                // Eq.(17)
+  const double E2 = 1.5 * fabs(dAp * (norm2(dz) / (dth2 * fabs(dotp(pA, pB))) - 1.0));
+  const double E3 = 0.1 * fabs(dAp) * dth2;
+  const double E4 = fabs(p1 - p2);
+  err += (E1 + E2) + (E3 + E4);
+}
+
+TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth) {
+  Piece P;
+  P.dA = 0.0;
+  P.err = 0.0;
+  P.crossing = 0;
+  const bool a5 = A.nreal() == 5, b5 = B.nreal() == 5;
+  int leftApos = -1, leftAneg = -1, leftBpos = -1, leftBneg = -1;
+  // ---- positive parity: slots 0,(1) --------------------------------------------------------------------
+  {
+    const cd A0 = A.z(0), B0 = B.z(0);
+    if (!a5 && !b5) {
+      link_terms(A, B, 0, 0, 1.0, dth, P.dA, P.err);
+    } else if (a5 && b5) {
+      const cd A1 = A.z(1), B1 = B.z(1);
+      const double straight = sqrt(norm2(A0 - B0)) + sqrt(norm2(A1 - B1));
+      const double crossed = sqrt(norm2(A0 - B1)) + sqrt(norm2(A1 - B0));
+      const int sw = crossed < straight;
+      link_terms(A, B, 0, sw, 1.0, dth, P.dA, P.err);
+      link_terms(A, B, 1, 1 - sw, 1.0, dth, P.dA, P.err);
+    } else if (b5) {   // 1 -> 2: the nearer one links, the other is left over
+      const int j = norm2(A0 - B.z(1)) < norm2(A0 - B0);
+      link_terms(A, B, 0, j, 1.0, dth, P.dA, P.err);
+      leftBpos = 1 - j;
+    } else {           // 2 -> 1
+      const int i = norm2(A.z(1) - B0) < norm2(A0 - B0);
+      link_terms(A, B, i, 0, 1.0, dth, P.dA, P.err);
+      leftApos = 1 - i;
+    }
+  }
+  // ---- negative parity: slots 2,3,(4): minimum-total-distance injective matching -----------------
+  {
+    const int na = a5 ? 3 : 2, nb = b5 ? 3 : 2;
+    double D[3][3];
+    cd za[3], zb[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      za[i] = (i < na) ? A.z(2 + i) : mk(0.0, 0.0);
+      zb[i] = (i < nb) ? B.z(2 + i) : mk(0.0, 0.0);
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        const bool ra = i < na, rb = j < nb;
+        // a missing third image is a dummy: free against real images when only one side lacks it, and forced
+        // onto the other dummy when both sides lack it
+        D[i][j] = (ra && rb) ? sqrt(norm2(za[i] - zb[j])) : ((ra || rb) ? ((na == nb) ? 1e300 : 0.0) : 0.0);
+      }
+    const int perm[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
+    int bestp = 0;
+    double best = D[0][0] + D[1][1] + D[2][2];
+#pragma unroll
+    for (int p = 1; p < 6; ++p) {
+      const double cost = D[0][perm[p][0]] + D[1][perm[p][1]] + D[2][perm[p][2]];
+      if (cost < best) { best = cost; bestp = p; }
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      int j = 0;
+#pragma unroll
+      for (int p = 0; p < 6; ++p)
+        if (p == bestp) j = perm[p][i];
+      const bool ra = i < na, rb = j < nb;
+      if (ra && rb) link_terms(A, B, 2 + i, 2 + j, -1.0, dth, P.dA, P.err);
+      else if (ra) leftAneg = 2 + i;
+      else if (rb) leftBneg = 2 + j;
+    }
+  }
+  // ---- caustic crossing: the extra (+,-) pair on the 5-image side connects to itself -------------
+  if (a5 != b5) {
+    const bool creation = b5;
+    const RecRef& S = creation ? B : A;
+    const int kp = creation ? leftBpos : leftApos;
+    const int km = creation ? leftBneg : leftAneg;
+    const cd zpl = S.z(kp), zmi = S.z(km), ppl = S.zp(kp), pmi = S.zp(km);
+    const double wpl = S.w(kp), wmi = S.w(km);
+    const cd d = zpl - zmi;
+    const double ad = sqrt(norm2(d));
+    const double sq = sqrt(fabs(dotp(ppl, pmi)));
+    const double dtt = ad / sq;                                         // Eq.(11) tilde Delta theta
+    const double dtt3 = dtt * dtt * dtt;
+    const double corr = (wpl - wmi) * dtt3 * (1.0 / 24.0);              // Eq.(11)
+    const double dd = dotp(d, ppl - pmi);
+    double chord, dAp, E2;
+    if (creation) {   // path z- -> z+, correction enters with '-' (S-2)
+      chord = 0.5 * wedge(zmi, d);
+      dAp = -corr;
+      E2 = 1.5 * fabs(dd - 2.0 * ad * sq) * dtt;                        // Eq.(18), reading E-5
+    } else {          // path z+ -> z-, correction enters with '+'
+      chord = -0.5 * wedge(zpl, d);
+      dAp = corr;
+      E2 = 1.5 * fabs(dd + 2.0 * ad * sq) * dtt;
+    }
+    P.crossing = creation ? 1 : -1;
+    P.dA += chord + dAp;
+    const double E1 = fabs(wpl + wmi) * dtt3 * (1.0 / 48.0);            // Eq.(18)
+    const double E3 = 0.1 * fabs(dAp) * dth * dth;
+    P.err += E1 + E2 + E3;
+  }
+  return P;
+}
+
+}  // namespace twk

@@ -1,0 +1,225 @@
+// twk_device.cuh -- device functions of the hot path, rows a1-a7 of SURVEY.md section 8(a).
+//
+//   a1  boundary sample            zeta_j = zeta_c + rho e^{i theta_j}, zeta'_j = i rho e^{i theta_j}
+//   a2  coefficient builder        Eq.(6), planet frame
+//   a3  quintic solve              Laguerre + forward deflation + Newton polish on the full polynomial
+//   a4  per-root lens quantities   f', f'', R (Eq.12), J (Eq.7), z' and z'^z'' (Eq.10, repaired)
+//   a5  ghost filter               residual detector, 2-cycle reading
+//   a6  contour linker             per-parity minimum-total-distance matching, creation / annihilation
+//   a7  area + error per interval  Eq.(9)-(11), Eq.(17)-(18)
+//
+// "P:<n>" = /root/reference/PAPER.md line n.  Nothing here is shared with oracle/ (which uses a different
+// root finder and enumerates permutations with the standard library).
+//
+// TWK_HD is __device__ in the product build.  (A host build of these functions exists only in throw-away
+// probes, never in the library.)
+#pragma once
+
+#include <math.h>
+#include <stdint.h>
+
+#ifndef TWK_HD
+#define TWK_HD __device__ __forceinline__
+#endif
+
+namespace twk {
+
+// ------------------------------------------------------------------------------------------------------------
+// complex FP64 arithmetic on register pairs
+// ------------------------------------------------------------------------------------------------------------
+struct cd {
+  double x, y;
+};
+TWK_HD cd mk(double x, double y) { cd r; r.x = x; r.y = y; return r; }
+TWK_HD cd operator+(cd a, cd b) { return mk(a.x + b.x, a.y + b.y); }
+TWK_HD cd operator-(cd a, cd b) { return mk(a.x - b.x, a.y - b.y); }
+TWK_HD cd operator-(cd a) { return mk(-a.x, -a.y); }
+TWK_HD cd operator*(cd a, cd b) { return mk(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x)); }
+TWK_HD cd operator*(double s, cd a) { return mk(s * a.x, s * a.y); }
+TWK_HD cd conj(cd a) { return mk(a.x, -a.y); }
+TWK_HD double norm2(cd a) { return fma(a.x, a.x, a.y * a.y); }
+TWK_HD double abs1(cd a) { return fabs(a.x) + fabs(a.y); }
+TWK_HD double wedge(cd a, cd b) { return fma(a.x, b.y, -(a.y * b.x)); }
+TWK_HD double dotp(cd a, cd b) { return fma(a.x, b.x, a.y * b.y); }
+TWK_HD cd cfma(cd a, cd b, cd c) {                                        // a*b + c
+  return mk(fma(a.x, b.x, fma(-a.y, b.y, c.x)), fma(a.x, b.y, fma(a.y, b.x, c.y)));
+}
+TWK_HD cd crecip(cd a) {
+  const double inv = 1.0 / norm2(a);
+  return mk(a.x * inv, -a.y * inv);
+}
+TWK_HD cd cdiv(cd a, cd b) {
+  const double inv = 1.0 / norm2(b);
+  return mk(fma(a.x, b.x, a.y * b.y) * inv, fma(a.y, b.x, -(a.x * b.y)) * inv);
+}
+TWK_HD cd csqrt_(cd a) {   // principal square root
+  const double r = sqrt(norm2(a));
+  if (r == 0.0) return mk(0.0, 0.0);
+  const double t = sqrt(0.5 * (r + fabs(a.x)));
+  const double u = 0.5 * a.y / t;
+  return (a.x >= 0.0) ? mk(t, u) : mk(fabs(u), copysign(t, a.y));
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// lens geometry, Eq.(2)
+// ------------------------------------------------------------------------------------------------------------
+struct Lens {
+  double s, m1, m2, z2;   // separation, masses normalised to the total, secondary position (CM frame)
+};
+TWK_HD Lens make_lens(double s, double q) {
+  Lens L;
+  const double inv = 1.0 / (1.0 + q);
+  L.s = s;
+  L.m1 = inv;
+  L.m2 = q * inv;
+  L.z2 = s * inv;
+  return L;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a2. Eq.(6): cancellation-free coefficients in the planet frame (planet at 0, primary at -s).
+//     y = zeta - z2, v_c = conj(y) + s, v_p = 1 + s conj(y).
+// ------------------------------------------------------------------------------------------------------------
+TWK_HD void coeffs_eq6(cd y, double s, double m2, cd c[6]) {
+  const cd yb = conj(y);
+  const cd vc = mk(yb.x + s, yb.y);
+  const cd vp = mk(fma(s, yb.x, 1.0), s * yb.y);
+  const double Iy = y.y;
+  const double m2s = m2 * s;
+  const double yy = norm2(y);   // conj(y) y
+  // c5 = -conj(y) v_c
+  c[5] = -(yb * vc);
+  // c4 = (conj(y) y - 1 - 2 s conj(y)) v_c + m2 s
+  {
+    const cd t = mk(yy - 1.0 - 2.0 * s * yb.x, -2.0 * s * yb.y);
+    const cd u = t * vc;
+    c[4] = mk(u.x + m2s, u.y);
+  }
+  // c3 = (2y - s) [v_p v_c + 2 i Im y - m2 s] + 4 i (m2 s - y) Im y
+  {
+    const cd a = mk(2.0 * y.x - s, 2.0 * y.y);
+    cd b = vp * vc;
+    b.x -= m2s;
+    b.y += 2.0 * Iy;
+    const cd d = mk(m2s - y.x, -y.y);           // (m2 s - y)
+    const cd e = mk(-4.0 * Iy * d.y, 4.0 * Iy * d.x);   // 4 i Im(y) (m2 s - y)
+    c[3] = a * b + e;
+  }
+  // c2 = Re(v_p)^2 Re(v_c) + i Im(y) Re(v_p) Re(1 - s y) + s Im(y)^2 (2 + s v_c) + m2 s [2 conj(y)(y - s) - (1 - s y)]
+  {
+    const double rvp = vp.x, rvc = vc.x;
+    const cd t3 = mk(2.0 + s * vc.x, s * vc.y);
+    const cd ys = mk(y.x - s, y.y);
+    const cd br = 2.0 * (yb * ys) - mk(1.0 - s * y.x, -s * y.y);
+    c[2] = mk(rvp * rvp * rvc + s * Iy * Iy * t3.x + m2s * br.x,
+              Iy * rvp * (1.0 - s * y.x) + s * Iy * Iy * t3.y + m2s * br.y);
+  }
+  // c1 = m2 s [(s + 2y) v_p + s (2 i s Im y - m2)]
+  {
+    const cd a = mk(s + 2.0 * y.x, 2.0 * y.y);
+    cd t = a * vp;
+    t.x += -s * m2;
+    t.y += 2.0 * s * s * Iy;
+    c[1] = m2s * t;
+  }
+  // c0 = s^2 m2^2 y
+  c[0] = (m2s * m2s) * y;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a3. quintic roots.  Laguerre iteration from x = 0 on the successively (forward-)deflated polynomial for the
+// first three roots, closed form for the remaining quadratic, then Newton steps on the ORIGINAL polynomial for
+// all five (removes deflation error).  All in registers; loops are compile-time bounded.
+// ------------------------------------------------------------------------------------------------------------
+constexpr double kEps = 2.220446049250313e-16;
+
+template <int N>
+TWK_HD cd laguerre(const cd (&a)[N + 1], cd x) {
+  double a1[N + 1];
+#pragma unroll
+  for (int i = 0; i <= N; ++i) a1[i] = abs1(a[i]);
+  double last = 1e300;
+  for (int it = 0; it < 48; ++it) {
+    cd p = a[N], d = mk(0.0, 0.0), h = mk(0.0, 0.0);   // p, p', p''/2
+    double err = a1[N];
+    const double ax = abs1(x);
+#pragma unroll
+    for (int i = N - 1; i >= 0; --i) {
+      h = cfma(h, x, d);
+      d = cfma(d, x, p);
+      p = cfma(p, x, a[i]);
+      err = fma(err, ax, a1[i]);
+    }
+    if (abs1(p) <= 2.0 * kEps * err) break;           // at the rounding floor of the evaluation
+    // dx = N p / (p' +- sqrt((N-1)((N-1) p'^2 - 2 N p p''/2)))
+    const cd g2 = d * d;
+    const cd ph = p * h;
+    const cd rad = mk(double(N - 1) * (double(N - 1) * g2.x - double(2 * N) * ph.x),
+                      double(N - 1) * (double(N - 1) * g2.y - double(2 * N) * ph.y));
+    cd sq = csqrt_(rad);
+    if (dotp(d, sq) < 0.0) sq = -sq;
+    const cd den = d + sq;
+    cd dx;
+    if (norm2(den) > 0.0) dx = cdiv(double(N) * p, den);
+    else dx = mk((1.0 + ax) * cos(double(it + 1)), (1.0 + ax) * sin(double(it + 1)));
+    const double sdx = abs1(dx);
+    if ((it & 7) == 7 && sdx >= last) dx = 0.5 * dx;   // break rare limit cycles
+    last = sdx;
+    x = x - dx;
+    if (sdx <= kEps * abs1(x)) break;
+  }
+  return x;
+}
+
+template <int N>
+TWK_HD void deflate(const cd (&a)[N + 1], cd r, cd (&b)[N]) {
+  b[N - 1] = a[N];
+#pragma unroll
+  for (int i = N - 1; i >= 1; --i) b[i - 1] = cfma(r, b[i], a[i]);
+}
+
+TWK_HD void quadratic(const cd (&a)[3], cd& r0, cd& r1) {
+  const cd disc = a[1] * a[1] - 4.0 * (a[2] * a[0]);
+  cd sq = csqrt_(disc);
+  if (dotp(a[1], sq) < 0.0) sq = -sq;
+  const cd qq = -0.5 * (a[1] + sq);
+  if (norm2(qq) > 0.0) {
+    r0 = cdiv(qq, a[2]);
+    r1 = cdiv(a[0], qq);
+  } else {
+    r0 = mk(0.0, 0.0);
+    r1 = mk(0.0, 0.0);
+  }
+}
+
+TWK_HD void quintic_roots(const cd (&c)[6], cd (&r)[5]) {
+  cd b4[5], b3[4], b2[3];
+  r[0] = laguerre<5>(c, mk(0.0, 0.0));
+  deflate<5>(c, r[0], b4);
+  r[1] = laguerre<4>(b4, mk(0.0, 0.0));
+  deflate<4>(b4, r[1], b3);
+  r[2] = laguerre<3>(b3, mk(0.0, 0.0));
+  deflate<3>(b3, r[2], b2);
+  quadratic(b2, r[3], r[4]);
+  // Newton polish on the undeflated quintic: two steps per root, five independent chains (ILP)
+#pragma unroll
+  for (int pass = 0; pass < 2; ++pass) {
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      cd p = c[5], d = mk(0.0, 0.0);
+#pragma unroll
+      for (int i = 4; i >= 0; --i) {
+        d = cfma(d, r[k], p);
+        p = cfma(p, r[k], c[i]);
+      }
+      const double dn = norm2(d);
+      if (dn > 0.0) {
+        const cd dx = cdiv(p, d);
+        // never let a polish step move a root by more than its own size (guards a vanishing p')
+        if (norm2(dx) <= norm2(r[k]) + 1e-300) r[k] = r[k] - dx;
+      }
+    }
+  }
+}
+
+}  // namespace twk

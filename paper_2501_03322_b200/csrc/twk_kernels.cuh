@@ -1,0 +1,193 @@
+// twk_kernels.cuh -- the kernels of the hot path (rows a8, a9 of SURVEY.md section 8(a) on top of the device
+// functions a1-a7 in twk_device.cuh / twk_contour.cuh).
+//
+//   fixed_kernel      fixed-sampling mode: theta_j = 2 pi j / N, one CTA per source, records staged in shared memory
+//   adaptive_kernel   the adaptive loop of P:318-326 for one source per 64-thread CTA, entirely on-device:
+//                     64 samples per iteration (one thread each), per-source sorted sample state in shared memory,
+//                     error-weighted inverse-transform sampling, stop rule + cap.
+//                     Stage 1 (kStage1): cap = 64, records in shared memory, every source of the batch;
+//                     stages 2/3: larger caps, records in a per-CTA global arena (L2 resident), sources taken
+//                     from the compacted worklist of the previous stage.
+//   compact_kernel    a9: worklist of unfinished sources by warp ballot + prefix sum
+//   dfma_probe_kernel FP64 FMA throughput probe (roofline denominator)
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include "twk_contour.cuh"
+
+namespace twk {
+
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+constexpr double kPi = 3.141592653589793238462643383279;
+constexpr int kThreads = 64;   // threads per source = samples per iteration
+
+struct Batch {
+  const double* s;
+  const double* q;
+  const double* rho;
+  const int32_t* model_id;   // may be null
+  const double* zeta;        // [n][2]
+  long long n_models, n_sources;
+};
+
+struct SourceParams {
+  Lens L;
+  cd zc;
+  double rho;
+  uint32_t status;   // TWK_ST_DOMAIN preset when outside P:374's range
+  bool valid;
+};
+
+__device__ __forceinline__ SourceParams load_source(const Batch& b, long long src) {
+  SourceParams P;
+  const long long m = b.model_id ? (long long)b.model_id[src] : (b.n_models == 1 ? 0 : src);
+  const double s = b.s[m], q = b.q[m], rho = b.rho[m];
+  P.zc = mk(b.zeta[2 * src], b.zeta[2 * src + 1]);
+  P.rho = rho;
+  P.valid = (s > 0.0) && (q > 0.0) && (rho > 0.0) && isfinite(s) && isfinite(q) && isfinite(rho) && isfinite(P.zc.x) &&
+            isfinite(P.zc.y) && m >= 0 && m < b.n_models;
+  P.status = (P.valid && s >= 0.1 && s <= 10.0 && q >= 1e-9) ? 0u : 8u;
+  P.L = make_lens(P.valid ? s : 1.0, P.valid ? q : 1.0);
+  return P;
+}
+
+// block-wide sum of two doubles over kThreads (2 warps) -- result valid in every thread
+__device__ __forceinline__ void block_sum2(double& a, double& b, double* scratch /* >= 4 doubles */) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    a += __shfl_xor_sync(0xffffffffu, a, o);
+    b += __shfl_xor_sync(0xffffffffu, b, o);
+  }
+  const int warp = threadIdx.x >> 5;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) {
+    scratch[2 * warp] = a;
+    scratch[2 * warp + 1] = b;
+  }
+  __syncthreads();
+  a = scratch[0] + scratch[2];
+  b = scratch[1] + scratch[3];
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Fixed-sampling mode.  TILE threads; records of one tile of samples in shared memory ([26][TILE]); the interval
+// (j-1 -> j) is evaluated by the thread of sample j, with the previous tile's last record carried over.
+// ------------------------------------------------------------------------------------------------------------
+template <int TILE>
+__global__ void __launch_bounds__(TILE) fixed_kernel(Batch b, int N, double* __restrict__ out_z, int8_t* __restrict__ out_kind,
+                                                     int8_t* __restrict__ out_count, double* __restrict__ out_mu,
+                                                     double* __restrict__ out_err) {
+  extern __shared__ double sm[];
+  double* rec = sm;                          // [26][TILE]
+  double* carry = rec + kRecDoubles * TILE;  // [26] last record of the previous tile
+  double* first = carry + kRecDoubles;       // [26] record of sample 0
+  double* red = first + kRecDoubles;         // [2 * TILE/32]
+  const int t = threadIdx.x;
+  for (long long src = blockIdx.x; src < b.n_sources; src += gridDim.x) {
+    const SourceParams S = load_source(b, src);
+    if (!S.valid) {
+      if (t == 0) {
+        if (out_mu) out_mu[src] = nan("");
+        if (out_err) out_err[src] = nan("");
+      }
+      continue;
+    }
+    double accA = 0.0, accE = 0.0;
+    const double dth = kTwoPi / double(N);
+    for (int base = 0; base < N; base += TILE) {
+      const int j = base + t;
+      const RecRef mine{rec + t, TILE};
+      if (j < N) {
+        const size_t o = (size_t)src * N + j;
+        point_solve(S.L, S.zc, S.rho, kTwoPi * double(j) / double(N), mine, out_z ? out_z + o * 10 : nullptr,
+                    out_kind ? out_kind + o * 5 : nullptr, out_count ? out_count + o : nullptr);
+      }
+      __syncthreads();
+      if (j < N && j >= 1) {
+        const RecRef prev = (t > 0) ? RecRef{rec + t - 1, TILE} : RecRef{carry, 1};
+        const Piece P = eval_interval(prev, mine, dth);
+        accA += P.dA;
+        accE += P.err;
+      }
+      __syncthreads();
+      if (j < N && (t == TILE - 1 || j == N - 1))
+        for (int e = 0; e < kRecDoubles; ++e) carry[e] = mine.at(e);
+      if (j == 0)
+        for (int e = 0; e < kRecDoubles; ++e) first[e] = mine.at(e);
+    }
+    __syncthreads();
+    if (t == 0) {   // closing interval (N-1 -> 0)
+      const Piece P = eval_interval(RecRef{carry, 1}, RecRef{first, 1}, dth);
+      accA += P.dA;
+      accE += P.err;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      accA += __shfl_xor_sync(0xffffffffu, accA, o);
+      accE += __shfl_xor_sync(0xffffffffu, accE, o);
+    }
+    if ((t & 31) == 0) {
+      red[2 * (t >> 5)] = accA;
+      red[2 * (t >> 5) + 1] = accE;
+    }
+    __syncthreads();
+    if (t == 0) {
+      double A = 0.0, E = 0.0;
+      for (int w = 0; w < TILE / 32; ++w) {
+        A += red[2 * w];
+        E += red[2 * w + 1];
+      }
+      if (out_mu) out_mu[src] = A / (kPi * S.rho * S.rho);
+      if (out_err) out_err[src] = E / fabs(A);
+    }
+    __syncthreads();
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// a9. worklist compaction: ids of sources with pending[i] != 0, by warp ballot + prefix sum.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) compact_kernel(const uint8_t* __restrict__ pending, long long n, int32_t* __restrict__ list,
+                                                      int* __restrict__ count) {
+  __shared__ int warp_tot[8];
+  __shared__ int block_base;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (long long base = (long long)blockIdx.x * 256; base < n; base += (long long)gridDim.x * 256) {
+    const long long i = base + threadIdx.x;
+    const bool p = (i < n) && pending[i];
+    const unsigned bal = __ballot_sync(0xffffffffu, p);
+    const int within = __popc(bal & ((1u << lane) - 1u));
+    if (lane == 0) warp_tot[warp] = __popc(bal);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int tot = 0;
+      for (int w = 0; w < 8; ++w) {
+        const int c = warp_tot[w];
+        warp_tot[w] = tot;
+        tot += c;
+      }
+      block_base = tot ? atomicAdd(count, tot) : 0;
+    }
+    __syncthreads();
+    if (p) list[block_base + warp_tot[warp] + within] = (int32_t)i;
+    __syncthreads();
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// FP64 FMA throughput probe: 8 independent DFMA chains per thread.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dfma_probe_kernel(int iters, double* __restrict__ out) {
+  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 1e-3, a2 = a0 + 2e-3, a3 = a0 + 3e-3, a4 = a0 + 4e-3, a5 = a0 + 5e-3,
+         a6 = a0 + 6e-3, a7 = a0 + 7e-3;
+  const double m = 0.999999, c = 1e-7;
+  for (int i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  const double sum = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (sum == 123.456) out[0] = sum;   // never true; keeps the chains alive
+}
+
+}  // namespace twk
