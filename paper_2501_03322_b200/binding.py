@@ -17,7 +17,7 @@ _lib = None
 TWK_ST_CONVERGED, TWK_ST_CAP, TWK_ST_REPAIRED, TWK_ST_DOMAIN, TWK_ST_NUMERIC = 1, 2, 4, 8, 16
 
 SYMBOLS = ["twk_default_options", "twk_create", "twk_destroy", "twk_workspace_bytes", "twk_magnify", "twk_images_fixed",
-           "twk_magnify_host", "twk_last_stats", "twk_fp64_peak_probe", "twk_strerror", "twk_version"]
+           "twk_magnify_host", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_strerror", "twk_version"]
 
 
 class TwkError(RuntimeError):
@@ -52,6 +52,8 @@ def lib():
         L.twk_magnify_host.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
         L.twk_images_fixed.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, vp]
         L.twk_last_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int), vp]
+        L.twk_enable_stage_timing.argtypes = [vp, i32]
+        L.twk_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.twk_fp64_peak_probe.argtypes = [i32, C.POINTER(dbl)]
         L.twk_strerror.argtypes = [i32]
         L.twk_strerror.restype = C.c_char_p
@@ -186,6 +188,14 @@ class Context:
         a, b, c = C.c_int64(), C.c_int64(), C.c_int()
         _check(lib().twk_last_stats(self._h, C.byref(a), C.byref(b), C.byref(c), _stream_ptr(stream)), "twk_last_stats")
         return dict(n_stage2=a.value, n_stage3=b.value, n_launches=c.value)
+
+    def twk_enable_stage_timing(self, on=True):
+        _check(lib().twk_enable_stage_timing(self._h, 1 if on else 0), "twk_enable_stage_timing")
+
+    def twk_last_stage_ms(self):
+        ms = (C.c_float * 4)()
+        _check(lib().twk_last_stage_ms(self._h, ms), "twk_last_stage_ms")
+        return dict(stage1=ms[0], compact=ms[1], stage2=ms[2], stage3=ms[3])
 
     # -- convenience over a workloads.Workload ------------------------------------------------------------------------
     def upload(self, wl, device="cuda"):

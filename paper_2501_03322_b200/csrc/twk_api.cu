@@ -82,6 +82,9 @@ struct twk_ctx {
   char* stage;
   size_t stage_bytes;
   int last_launches;
+  int timing;            // record CUDA events around every stage (twk_enable_stage_timing)
+  cudaEvent_t ev[5];     // start, after stage 1, after compaction, after stage 2, after stage 3
+  int ev_used;           // number of events recorded by the last call
 };
 
 extern "C" {
@@ -123,16 +126,19 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   c->stage = nullptr;
   c->stage_bytes = 0;
   c->last_launches = 0;
+  c->timing = 0;
+  c->ev_used = 0;
+  for (int i = 0; i < 5; ++i) c->ev[i] = nullptr;
   cudaError_t e = cudaMalloc((void**)&c->ws, c->lay.total);
   if (e != cudaSuccess) {
     delete c;
     cudaGetLastError();
     return e == cudaErrorMemoryAllocation ? TWK_ENOMEM : cuda_fail(e);
   }
-  // opt in to the large dynamic shared memory of stage 3
-  const int cap_big = c->plan.cap3 ? c->plan.cap3 : (c->plan.cap2 ? c->plan.cap2 : twk::kThreads);
+  // opt in to the large dynamic shared memory of stage 3 (a per-function attribute shared by all contexts, so
+  // always the maximum the build supports)
   e = cudaFuncSetAttribute(twk::adaptive_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)twk::adaptive_smem_bytes(cap_big, false));
+                           (int)twk::adaptive_smem_bytes(4096, false));
   if (e != cudaSuccess) {
     cudaFree(c->ws);
     delete c;
@@ -146,6 +152,8 @@ int twk_destroy(twk_ctx* ctx) {
   if (!ctx) return TWK_OK;
   if (ctx->ws) cudaFree(ctx->ws);
   if (ctx->stage) cudaFree(ctx->stage);
+  for (int i = 0; i < 5; ++i)
+    if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
   delete ctx;
   return TWK_OK;
 }
@@ -185,6 +193,11 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
   int32_t* list1 = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list1);
   int32_t* list2 = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list2);
   int launches = 0;
+  ctx->ev_used = 0;
+  auto mark = [&]() {
+    if (ctx->timing && ctx->ev_used < 5) cudaEventRecord(ctx->ev[ctx->ev_used++], stream);
+  };
+  mark();
   // ---- stage 1: every source, 64 samples, records in shared memory ------------------------------------------------
   {
     twk::AdaptArgs a1 = a;
@@ -197,6 +210,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     const int grid = (int)((long long)n_sources < resident ? (long long)n_sources : resident);
     twk::adaptive_kernel<true><<<grid, twk::kThreads, twk::adaptive_smem_bytes(twk::kThreads, true), stream>>>(a1);
     ++launches;
+    mark();
   }
   if (P.cap2) {
     // ---- a9: compact the unfinished sources (ballot + prefix sum) ---------------------------------------------------
@@ -204,6 +218,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     const int grid = (int)(blocks < 4096 ? blocks : 4096);
     twk::compact_kernel<<<grid, 256, 0, stream>>>(a.pending, (long long)n_sources, list1, counters + 1);
     ++launches;
+    mark();
     // ---- stage 2 -----------------------------------------------------------------------------------------------------
     twk::AdaptArgs a2 = a;
     a2.cap = P.cap2;
@@ -215,6 +230,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     a2.next_count = counters + 3;
     twk::adaptive_kernel<false><<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2, false), stream>>>(a2);
     ++launches;
+    mark();
   }
   if (P.cap3) {
     twk::AdaptArgs a3 = a;
@@ -225,6 +241,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     a3.cursor = counters + 4;
     twk::adaptive_kernel<false><<<P.grid3, twk::kThreads, twk::adaptive_smem_bytes(P.cap3, false), stream>>>(a3);
     ++launches;
+    mark();
   }
   ctx->last_launches = launches;
   TWK_CUDA(cudaGetLastError());
@@ -305,6 +322,25 @@ int twk_last_stats(twk_ctx* ctx, int64_t* n_stage2, int64_t* n_stage3, int* n_la
   if (n_stage2) *n_stage2 = h[1];
   if (n_stage3) *n_stage3 = h[3];
   if (n_launches) *n_launches = ctx->last_launches;
+  return TWK_OK;
+}
+
+int twk_enable_stage_timing(twk_ctx* ctx, int on) {
+  if (!ctx) return TWK_EINVAL;
+  if (on)
+    for (int i = 0; i < 5; ++i)
+      if (!ctx->ev[i]) TWK_CUDA(cudaEventCreate(&ctx->ev[i]));
+  ctx->timing = on ? 1 : 0;
+  ctx->ev_used = 0;
+  return TWK_OK;
+}
+
+int twk_last_stage_ms(twk_ctx* ctx, float* ms4) {
+  if (!ctx || !ms4) return TWK_EINVAL;
+  for (int i = 0; i < 4; ++i) ms4[i] = 0.0f;
+  if (!ctx->timing || ctx->ev_used < 2) return TWK_EINVAL;
+  TWK_CUDA(cudaEventSynchronize(ctx->ev[ctx->ev_used - 1]));
+  for (int i = 0; i + 1 < ctx->ev_used; ++i) TWK_CUDA(cudaEventElapsedTime(&ms4[i], ctx->ev[i], ctx->ev[i + 1]));
   return TWK_OK;
 }
 
