@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtwk.so")
 SOURCES = ["twk_api.cu"]
-HEADERS = ["twk_device.cuh", "twk_contour.cuh", "twk_kernels.cuh", "twk_adaptive.cuh"]
+HEADERS = ["twk_device.cuh", "twk_contour.cuh", "twk_kernels.cuh", "twk_adaptive.cuh", "twk_stage1.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "-shared", "-cudart", "shared"]
 

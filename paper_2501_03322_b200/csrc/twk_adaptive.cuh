@@ -1,4 +1,6 @@
-// twk_adaptive.cuh -- a8 + a9: the adaptive contour loop for one source per 64-thread CTA (see twk_kernels.cuh).
+// twk_adaptive.cuh -- a8 + a9: the adaptive contour loop for one source per 64-thread CTA (refinement stages 2 and 3;
+// see twk_kernels.cuh).  Boundary samples are solved by seeded Newton from the source centre's roots (thread 0 cold-
+// solves the centre once per source), with the cold solver as verified fallback.
 #pragma once
 
 #include "twk_kernels.cuh"
@@ -14,7 +16,6 @@ struct AdaptArgs {
   const int32_t* list;   // worklist of source ids (null: all sources 0..n_sources-1)
   const int* count;      // number of entries of `list` (device; null: n_sources)
   int* cursor;           // dynamic work fetch counter (device, zeroed before launch)
-  uint8_t* pending;      // stage 1 only: pending[src] = 1 when the source needs stage 2
   int32_t* next_list;    // stage 2 only: sources that need stage 3 ...
   int* next_count;       // ... appended with atomicAdd
   double* arena;         // stages 2/3: gridDim.x * cap records of kRecDoubles doubles
@@ -24,14 +25,13 @@ struct AdaptArgs {
   uint32_t* out_status;  // may be null
 };
 
-__host__ __device__ inline size_t adaptive_smem_bytes(int cap, bool stage1) {
-  size_t doubles = 3 * (size_t)cap + 2 * kThreads + 8 + (stage1 ? kRecDoubles * kThreads : 0);
+__host__ __device__ inline size_t adaptive_smem_bytes(int cap) {
+  size_t doubles = 3 * (size_t)cap + 2 * kThreads + 8 + 10;
   size_t ints = 2 * kThreads + 4;
   return doubles * 8 + ints * 4 + (size_t)cap * 2;
 }
 
-template <bool kStage1>
-__global__ void __launch_bounds__(kThreads, kStage1 ? 6 : 4) adaptive_kernel(AdaptArgs p) {
+__global__ void __launch_bounds__(kThreads, 4) adaptive_kernel(AdaptArgs p) {
   extern __shared__ double sm[];
   const int cap = p.cap;
   double* theta = sm;            // [cap] sorted sample angles
@@ -40,18 +40,16 @@ __global__ void __launch_bounds__(kThreads, kStage1 ? 6 : 4) adaptive_kernel(Ada
   double* newth = er + cap;      // [64]  angle of quantile k
   double* cth = newth + kThreads;   // [64] compacted new angles
   double* scratch = cth + kThreads; // [8]
-  double* recs = scratch + 8;       // stage 1: [26][64] records
-  int* newint = reinterpret_cast<int*>(recs + (kStage1 ? kRecDoubles * kThreads : 0));   // [64] interval of quantile k
+  double* seeds = scratch + 8;      // [10] planet-frame roots of the source centre (Re x5, Im x5)
+  int* newint = reinterpret_cast<int*>(seeds + 10);   // [64] interval of quantile k
   int* cint = newint + kThreads;    // [64] compacted
   int* iscr = cint + kThreads;      // [4]
   uint16_t* ids = reinterpret_cast<uint16_t*>(iscr + 4);   // [cap] arena id of the sample at each sorted position
 
   const int t = threadIdx.x;
   const int lane = t & 31, warp = t >> 5;
-  double* arena = kStage1 ? nullptr : p.arena + (size_t)blockIdx.x * (size_t)cap * kRecDoubles;
-  auto recref = [&](int id) -> RecRef {
-    return kStage1 ? RecRef{recs + id, kThreads} : RecRef{arena + (size_t)id * kRecDoubles, 1};
-  };
+  double* arena = p.arena + (size_t)blockIdx.x * (size_t)cap * kRecDoubles;
+  auto recref = [&](int id) -> RecRef { return RecRef{arena + (size_t)id * kRecDoubles, 1}; };
   const long long total = p.count ? (long long)*p.count : p.b.n_sources;
 
   for (;;) {
@@ -68,17 +66,28 @@ __global__ void __launch_bounds__(kThreads, kStage1 ? 6 : 4) adaptive_kernel(Ada
         if (p.out_err) p.out_err[src] = nan("");
         if (p.out_nsamples) p.out_nsamples[src] = 0;
         if (p.out_status) p.out_status[src] = 8u;
-        if (kStage1) p.pending[src] = 0;
       }
       continue;
     }
+    if (t == 0) {
+      cd eta[5];
+      centre_roots(S.L, S.zc, eta);
+#pragma unroll
+      for (int k = 0; k < 5; ++k) {
+        seeds[k] = eta[k].x;
+        seeds[5 + k] = eta[k].y;
+      }
+    }
+    __syncthreads();
     // ---- first iteration: 64 uniform samples theta_j = 2 pi j / 64 (reading A-3) ----------------------
     int flags = 0;
     {
       const double th = kTwoPi * double(t) / double(kThreads);
-      flags |= point_solve(S.L, S.zc, S.rho, th, recref(t), nullptr, nullptr, nullptr);
+      double sn, cs;
+      sincospi(double(t) / 32.0, &sn, &cs);
+      flags |= point_solve_cs(S.L, S.zc, S.rho, cs, sn, seeds, 1, recref(t), nullptr, nullptr, nullptr);
       theta[t] = th;
-      if (!kStage1) ids[t] = (uint16_t)t;
+      ids[t] = (uint16_t)t;
     }
     __syncthreads();
     {
@@ -105,7 +114,6 @@ __global__ void __launch_bounds__(kThreads, kStage1 ? 6 : 4) adaptive_kernel(Ada
       if (!(isfinite(A) && isfinite(E))) { status |= 16u; break; }
       if (E <= tolA) { status |= 1u; break; }                       // stop rule P:272, reading A-1
       if (n + kThreads > cap) { exhausted = true; break; }          // cap P:326, reading A-6
-      if (kStage1) { exhausted = true; break; }                     // (cap == 64: unreachable, lets the compiler drop the rest)
       // ---- a8: error-weighted inverse-transform sampling, 64 quantiles ---------------------------
       const double avg = p.subtract_avg_tol ? tolA / double(n) : 0.0;   // "average tolerance", reading A-5
       double W = 0.0, unused = 0.0;
@@ -198,7 +206,9 @@ __global__ void __launch_bounds__(kThreads, kStage1 ? 6 : 4) adaptive_kernel(Ada
         const double th = cth[t];
         theta[pos] = th;
         ids[pos] = (uint16_t)(n + t);
-        flags |= point_solve(S.L, S.zc, S.rho, th, recref(n + t), nullptr, nullptr, nullptr);
+        double sn, cs;
+        sincos(th, &sn, &cs);
+        flags |= point_solve_cs(S.L, S.zc, S.rho, cs, sn, seeds, 1, recref(n + t), nullptr, nullptr, nullptr);
       }
       const int n_new = n + m;
       __syncthreads();
@@ -225,8 +235,7 @@ __global__ void __launch_bounds__(kThreads, kStage1 ? 6 : 4) adaptive_kernel(Ada
     const int nonf = __syncthreads_or(flags & kPointNonFinite);
     if (t == 0) {
       if (exhausted && !p.final_stage) {
-        if (kStage1) p.pending[src] = 1;
-        else p.next_list[atomicAdd(p.next_count, 1)] = (int32_t)src;
+        p.next_list[atomicAdd(p.next_count, 1)] = (int32_t)src;
       } else {
         if (exhausted) status |= 2u;
         if (rep) status |= 4u;
@@ -235,7 +244,6 @@ __global__ void __launch_bounds__(kThreads, kStage1 ? 6 : 4) adaptive_kernel(Ada
         if (p.out_err) p.out_err[src] = E / fabs(A);
         if (p.out_nsamples) p.out_nsamples[src] = n;
         if (p.out_status) p.out_status[src] = status;
-        if (kStage1) p.pending[src] = 0;
       }
     }
   }

@@ -7,6 +7,7 @@
 
 #include "../../include/twk.h"
 #include "twk_adaptive.cuh"
+#include "twk_stage1.cuh"
 
 namespace {
 
@@ -137,8 +138,8 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   }
   // opt in to the large dynamic shared memory of stage 3 (a per-function attribute shared by all contexts, so
   // always the maximum the build supports)
-  e = cudaFuncSetAttribute(twk::adaptive_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)twk::adaptive_smem_bytes(4096, false));
+  e = cudaFuncSetAttribute(twk::adaptive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)twk::adaptive_smem_bytes(4096));
   if (e != cudaSuccess) {
     cudaFree(c->ws);
     delete c;
@@ -189,7 +190,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
   a.out_nsamples = out_nsamples;
   a.out_status = out_status;
   a.arena = reinterpret_cast<double*>(ctx->ws + ctx->lay.arena);
-  a.pending = reinterpret_cast<uint8_t*>(ctx->ws + ctx->lay.pending);
+  uint8_t* pending = reinterpret_cast<uint8_t*>(ctx->ws + ctx->lay.pending);
   int32_t* list1 = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list1);
   int32_t* list2 = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list2);
   int launches = 0;
@@ -198,17 +199,22 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     if (ctx->timing && ctx->ev_used < 5) cudaEventRecord(ctx->ev[ctx->ev_used++], stream);
   };
   mark();
-  // ---- stage 1: every source, 64 samples, records in shared memory ------------------------------------------------
+  // ---- stage 1: every source, 64 samples, groups of 64 sources per CTA, everything in shared memory ----------------
   {
-    twk::AdaptArgs a1 = a;
-    a1.cap = twk::kThreads;
+    twk::Stage1Args a1{};
+    a1.b = a.b;
+    a1.tol = rel_tol;
     a1.final_stage = P.cap2 ? 0 : 1;
-    a1.list = nullptr;
-    a1.count = nullptr;
     a1.cursor = counters + 0;
+    a1.pending = pending;
+    a1.out_mu = out_mu;
+    a1.out_err = out_err;
+    a1.out_nsamples = out_nsamples;
+    a1.out_status = out_status;
+    const long long groups = ((long long)n_sources + twk::kThreads - 1) / twk::kThreads;
     const long long resident = (long long)ctx->sms * 6;
-    const int grid = (int)((long long)n_sources < resident ? (long long)n_sources : resident);
-    twk::adaptive_kernel<true><<<grid, twk::kThreads, twk::adaptive_smem_bytes(twk::kThreads, true), stream>>>(a1);
+    const int grid = (int)(groups < resident ? groups : resident);
+    twk::stage1_kernel<<<grid, twk::kThreads, twk::stage1_smem_bytes(), stream>>>(a1);
     ++launches;
     mark();
   }
@@ -216,7 +222,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     // ---- a9: compact the unfinished sources (ballot + prefix sum) ---------------------------------------------------
     const long long blocks = ((long long)n_sources + 255) / 256;
     const int grid = (int)(blocks < 4096 ? blocks : 4096);
-    twk::compact_kernel<<<grid, 256, 0, stream>>>(a.pending, (long long)n_sources, list1, counters + 1);
+    twk::compact_kernel<<<grid, 256, 0, stream>>>(pending, (long long)n_sources, list1, counters + 1);
     ++launches;
     mark();
     // ---- stage 2 -----------------------------------------------------------------------------------------------------
@@ -228,7 +234,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     a2.cursor = counters + 2;
     a2.next_list = list2;
     a2.next_count = counters + 3;
-    twk::adaptive_kernel<false><<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2, false), stream>>>(a2);
+    twk::adaptive_kernel<<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2), stream>>>(a2);
     ++launches;
     mark();
   }
@@ -239,7 +245,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     a3.list = list2;
     a3.count = counters + 3;
     a3.cursor = counters + 4;
-    twk::adaptive_kernel<false><<<P.grid3, twk::kThreads, twk::adaptive_smem_bytes(P.cap3, false), stream>>>(a3);
+    twk::adaptive_kernel<<<P.grid3, twk::kThreads, twk::adaptive_smem_bytes(P.cap3), stream>>>(a3);
     ++launches;
     mark();
   }

@@ -38,16 +38,23 @@ constexpr int kPointNonFinite = 2;  // a root or a derived quantity is not finit
 // a1 + a2 + a3 + a4 + a5: one boundary point source.
 // Writes the record; optionally the five roots (CM frame), their kinds and the real-image count.
 // ------------------------------------------------------------------------------------------------------------
-TWK_HD int point_solve(const Lens& L, cd zc, double rho, double theta, RecRef rec, double* out_z, int8_t* out_kind,
-                       int8_t* out_count) {
-  double sn, cs;
-  sincos(theta, &sn, &cs);
+// cs, sn = cos(theta), sin(theta).  seeds: nullptr = cold solve; otherwise five planet-frame roots of a nearby point
+// source (element k at seeds[k * seed_stride] (re) and seeds[(5 + k) * seed_stride] (im)) for the seeded Newton
+// solve, with the cold solver as verified fallback.
+TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn, const double* seeds, int seed_stride,
+                          RecRef rec, double* out_z, int8_t* out_kind, int8_t* out_count) {
   const cd zeta = mk(fma(rho, cs, zc.x), fma(rho, sn, zc.y));
   const cd dzeta = mk(-rho * sn, rho * cs);                     // zeta' = i rho e^{i theta}
   const cd y = mk(zeta.x - L.z2, zeta.y);
   cd c[6], eta[5];
   coeffs_eq6(y, L.s, L.m2, c);
-  quintic_roots(c, eta);
+  bool solved = false;
+  if (seeds) {
+#pragma unroll
+    for (int k = 0; k < 5; ++k) eta[k] = mk(seeds[k * seed_stride], seeds[(5 + k) * seed_stride]);
+    solved = quintic_roots_seeded(c, eta);
+  }
+  if (!solved) quintic_roots(c, eta);
 
   // a4: f', f'', residual, Jacobian in the planet frame (z2 - z = -eta, z1 - z = -s - eta; both are frame
   // invariant)
@@ -136,6 +143,20 @@ TWK_HD int point_solve(const Lens& L, cd zc, double rho, double theta, RecRef re
   rec.at(kNR) = double(nreal + ((flags & kPointRepaired) ? 8 : 0));
   if (out_count) *out_count = (int8_t)nreal;
   return flags;
+}
+
+TWK_HD int point_solve(const Lens& L, cd zc, double rho, double theta, RecRef rec, double* out_z, int8_t* out_kind,
+                       int8_t* out_count) {
+  double sn, cs;
+  sincos(theta, &sn, &cs);
+  return point_solve_cs(L, zc, rho, cs, sn, nullptr, 0, rec, out_z, out_kind, out_count);
+}
+
+// Cold solve of the point source at the source CENTRE: its five planet-frame roots seed the boundary samples.
+TWK_HD void centre_roots(const Lens& L, cd zc, cd (&eta)[5]) {
+  cd c[6];
+  coeffs_eq6(mk(zc.x - L.z2, zc.y), L.s, L.m2, c);
+  quintic_roots(c, eta);
 }
 
 // ------------------------------------------------------------------------------------------------------------

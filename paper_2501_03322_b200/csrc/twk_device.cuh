@@ -222,4 +222,42 @@ TWK_HD void quintic_roots(const cd (&c)[6], cd (&r)[5]) {
   }
 }
 
+// Seeded solve: Newton iteration on the ORIGINAL quintic for all five roots at once (five independent chains),
+// started from the roots of a nearby point source (the source centre, or the neighbouring boundary sample).
+// Roots of a polynomial are continuous in its coefficients, so ghosts can be followed like real images.
+// Returns true when every root converged and the five are distinct (Vieta: sum of roots = -c4/c5); otherwise the
+// caller falls back to the cold solver quintic_roots().  r[] holds the seeds on entry and the roots on exit.
+TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5]) {
+  double c1[6];
+#pragma unroll
+  for (int i = 0; i < 6; ++i) c1[i] = abs1(c[i]);
+  unsigned done = 0;
+  for (int it = 0; it < 10 && done != 31u; ++it) {
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      cd p = c[5], d = mk(0.0, 0.0);
+      double err = c1[5];
+      const double ax = abs1(r[k]);
+#pragma unroll
+      for (int i = 4; i >= 0; --i) {
+        d = cfma(d, r[k], p);
+        p = cfma(p, r[k], c[i]);
+        err = fma(err, ax, c1[i]);
+      }
+      if (abs1(p) <= 2.0 * kEps * err) { done |= 1u << k; continue; }   // at the rounding floor
+      const double dn = norm2(d);
+      if (!(dn > 0.0)) continue;
+      const cd dx = cdiv(p, d);
+      r[k] = r[k] - dx;
+      if (abs1(dx) <= 1e-12 * abs1(r[k])) done |= 1u << k;
+    }
+  }
+  if (done != 31u) return false;
+  // distinctness: sum of the roots against -c4/c5
+  const cd want = -cdiv(c[4], c[5]);
+  const cd sum = (r[0] + r[1]) + (r[2] + r[3]) + r[4];
+  const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
+  return abs1(sum - want) <= 1e-9 * scale;
+}
+
 }  // namespace twk
