@@ -242,7 +242,6 @@ def main():
         s1 = float(np.mean([x["stage1"] for x in stage_ms]))
         s2 = float(np.mean([x["stage2"] for x in stage_ms]))
         s3 = float(np.mean([x["stage3"] for x in stage_ms]))
-        sc = float(np.mean([x["compact"] for x in stage_ms]))
         flop_launch = FLOP_PER_POINT * 64.0 * n                   # stage 1 solves 64 boundary points per source
         achieved = flop_launch / (s1 * 1e-3) / 1e12
         line = {
@@ -258,13 +257,13 @@ def main():
                     "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps},
             "gpu_launches": stats["n_launches"] * args.steps,
             "clocks": clocks,
-            "roofline": {"bound": "alu", "kernel": "adaptive_kernel<true> (stage 1: 64 point solves + 64 intervals per source)",
+            "roofline": {"bound": "alu", "kernel": "stage1_kernel (64 point solves + 64 intervals per source)",
                          "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf, "traffic": None,
                          "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x "
                                         f"{sm_max_mhz:.0f} MHz (MEASURED_PEAKS.json has no FP64 figure)",
                          "peak_probe_tflops": probe_tf, "frac_of_probe": achieved / probe_tf,
                          "flop_per_point": FLOP_PER_POINT, "points_per_launch": 64 * n,
-                         "kernel_ms": {"stage1": s1, "compact": sc, "stage2": s2, "stage3": s3},
+                         "kernel_ms": {"stage1": s1, "stage2": s2, "stage3": s3},
                          "stage1_share_of_step": s1 / (ms / args.steps),
                          "point_solves_per_s": total_points * args.steps / (ms * 1e-3)},
         }

@@ -51,6 +51,10 @@ typedef struct {
   int initial_samples;  /* uniform samples of the first iteration, default 64; must be 64 in this build    */
   int max_samples;      /* sample cap per source, default 4096; 64 <= max_samples <= 4096                  */
   int subtract_avg_tol; /* 1 = subtract the average tolerance from every interval error before sampling */
+  int64_t handoff_slots; /* slots of the hand-over arena through which the first iteration (64 records, interval     */
+                        /* pieces, seeds; 14,592 B per slot) of an unfinished source passes to the refinement stage  */
+                        /* instead of being recomputed there.  -1 = default min(max_sources, 524288); 0 = none.      */
+                        /* Sources beyond the slots are still refined (their first iteration is recomputed).        */
 } twk_options;
 
 /* Fill *opt with the defaults above. */
@@ -103,10 +107,10 @@ int twk_last_stats(twk_ctx* ctx, int64_t* n_stage2, int64_t* n_stage3, int* n_la
 
 /* Per-stage device timing of twk_magnify for measurement: when enabled, CUDA events are recorded on the call's
  * stream around each stage.  twk_last_stage_ms waits for the last recorded event and writes the durations (ms)
- * of {stage-1 kernel, compaction kernel, stage-2 kernel, stage-3 kernel} of the last twk_magnify on this context
- * (0 for absent stages) into ms4[4]. */
+ * of {stage-1 kernel, stage-2 kernel, stage-3 kernel} of the last twk_magnify on this context (0 for absent
+ * stages) into ms3[3]. */
 int twk_enable_stage_timing(twk_ctx* ctx, int on);
-int twk_last_stage_ms(twk_ctx* ctx, float* ms4);
+int twk_last_stage_ms(twk_ctx* ctx, float* ms3);
 
 /* FP64 FMA throughput probe used for the ALU roofline denominator: runs `iters` dependent-chain DFMAs per thread
  * (8 independent chains per thread, a full persistent grid) and returns the measured TFLOP/s (2 flop per DFMA) in

@@ -26,7 +26,7 @@ class TwkError(RuntimeError):
 
 class twk_options(C.Structure):
     _fields_ = [("samples_per_iter", C.c_int), ("initial_samples", C.c_int), ("max_samples", C.c_int),
-                ("subtract_avg_tol", C.c_int)]
+                ("subtract_avg_tol", C.c_int), ("handoff_slots", C.c_int64)]
 
 
 def library_path() -> str:
@@ -193,9 +193,9 @@ class Context:
         _check(lib().twk_enable_stage_timing(self._h, 1 if on else 0), "twk_enable_stage_timing")
 
     def twk_last_stage_ms(self):
-        ms = (C.c_float * 4)()
+        ms = (C.c_float * 3)()
         _check(lib().twk_last_stage_ms(self._h, ms), "twk_last_stage_ms")
-        return dict(stage1=ms[0], compact=ms[1], stage2=ms[2], stage3=ms[3])
+        return dict(stage1=ms[0], stage2=ms[1], stage3=ms[2])
 
     # -- convenience over a workloads.Workload ------------------------------------------------------------------------
     def upload(self, wl, device="cuda"):

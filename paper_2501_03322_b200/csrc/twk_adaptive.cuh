@@ -1,6 +1,8 @@
 // twk_adaptive.cuh -- a8 + a9: the adaptive contour loop for one source per 64-thread CTA (refinement stages 2 and 3;
-// see twk_kernels.cuh).  Boundary samples are solved by seeded Newton from the source centre's roots (thread 0 cold-
-// solves the centre once per source), with the cold solver as verified fallback.
+// see twk_kernels.cuh).  A stage-2 source normally arrives with its first iteration done: stage 1 handed over its 64
+// records, 64 interval pieces and seed block (hand-over arena), which are used in place.  Otherwise (no free
+// hand-over slot, or stage 3) the first iteration is recomputed here.  New samples are solved by seeded Newton from
+// the source centre's seed block, with the cold solver as verified fallback.
 #pragma once
 
 #include "twk_kernels.cuh"
@@ -19,6 +21,8 @@ struct AdaptArgs {
   int32_t* next_list;    // stage 2 only: sources that need stage 3 ...
   int* next_count;       // ... appended with atomicAdd
   double* arena;         // stages 2/3: gridDim.x * cap records of kRecDoubles doubles
+  const double* handoff; // stage 2: hand-over arena written by stage 1 (null: recompute the first iteration)
+  long long handoff_slots;   // worklist entries < handoff_slots have a hand-over slot
   double* out_mu;
   double* out_err;       // may be null
   int32_t* out_nsamples; // may be null
@@ -26,12 +30,12 @@ struct AdaptArgs {
 };
 
 __host__ __device__ inline size_t adaptive_smem_bytes(int cap) {
-  size_t doubles = 3 * (size_t)cap + 2 * kThreads + 8 + 10;
+  size_t doubles = 3 * (size_t)cap + 2 * kThreads + 8 + 32;
   size_t ints = 2 * kThreads + 4;
   return doubles * 8 + ints * 4 + (size_t)cap * 2;
 }
 
-__global__ void __launch_bounds__(kThreads, 4) adaptive_kernel(AdaptArgs p) {
+__global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   extern __shared__ double sm[];
   const int cap = p.cap;
   double* theta = sm;            // [cap] sorted sample angles
@@ -40,8 +44,8 @@ __global__ void __launch_bounds__(kThreads, 4) adaptive_kernel(AdaptArgs p) {
   double* newth = er + cap;      // [64]  angle of quantile k
   double* cth = newth + kThreads;   // [64] compacted new angles
   double* scratch = cth + kThreads; // [8]
-  double* seeds = scratch + 8;      // [10] planet-frame roots of the source centre (Re x5, Im x5)
-  int* newint = reinterpret_cast<int*>(seeds + 10);   // [64] interval of quantile k
+  double* seeds = scratch + 8;      // [30 (+2)] seed block of the source (twk_contour.cuh)
+  int* newint = reinterpret_cast<int*>(seeds + 32);   // [64] interval of quantile k
   int* cint = newint + kThreads;    // [64] compacted
   int* iscr = cint + kThreads;      // [4]
   uint16_t* ids = reinterpret_cast<uint16_t*>(iscr + 4);   // [cap] arena id of the sample at each sorted position
@@ -49,7 +53,12 @@ __global__ void __launch_bounds__(kThreads, 4) adaptive_kernel(AdaptArgs p) {
   const int t = threadIdx.x;
   const int lane = t & 31, warp = t >> 5;
   double* arena = p.arena + (size_t)blockIdx.x * (size_t)cap * kRecDoubles;
-  auto recref = [&](int id) -> RecRef { return RecRef{arena + (size_t)id * kRecDoubles, 1}; };
+  // record of sample id: ids 0..63 of a handed-over source live in its hand-over slot ([26][64]), the rest in the arena
+  const double* hand = nullptr;
+  auto recref = [&](int id) -> RecRef {
+    if (hand && id < kThreads) return RecRef{const_cast<double*>(hand) + id, kThreads};
+    return RecRef{arena + (size_t)id * kRecDoubles, 1};
+  };
   const long long total = p.count ? (long long)*p.count : p.b.n_sources;
 
   for (;;) {
@@ -69,28 +78,23 @@ __global__ void __launch_bounds__(kThreads, 4) adaptive_kernel(AdaptArgs p) {
       }
       continue;
     }
-    if (t == 0) {
-      cd eta[5];
-      centre_roots(S.L, S.zc, eta);
-#pragma unroll
-      for (int k = 0; k < 5; ++k) {
-        seeds[k] = eta[k].x;
-        seeds[5 + k] = eta[k].y;
-      }
-    }
-    __syncthreads();
     // ---- first iteration: 64 uniform samples theta_j = 2 pi j / 64 (reading A-3) ----------------------
     int flags = 0;
-    {
-      const double th = kTwoPi * double(t) / double(kThreads);
+    theta[t] = kTwoPi * double(t) / double(kThreads);
+    ids[t] = (uint16_t)t;
+    hand = (p.handoff && cur < p.handoff_slots) ? p.handoff + (size_t)cur * kHandDoubles : nullptr;
+    if (hand) {   // done by stage 1: take its interval pieces and seed block, use its records in place
+      dA[t] = hand[kRecDoubles * kThreads + t];
+      er[t] = hand[(kRecDoubles + 1) * kThreads + t];
+      if (t < kSeedDoubles) seeds[t] = hand[(kRecDoubles + 2) * kThreads + t];
+      flags |= recref(t).point_flags();
+    } else {
+      if (t == 0) centre_seeds(S.L, S.zc, S.rho, seeds, 1);
+      __syncthreads();
       double sn, cs;
       sincospi(double(t) / 32.0, &sn, &cs);
       flags |= point_solve_cs(S.L, S.zc, S.rho, cs, sn, seeds, 1, recref(t), nullptr, nullptr, nullptr);
-      theta[t] = th;
-      ids[t] = (uint16_t)t;
-    }
-    __syncthreads();
-    {
+      __syncthreads();
       const Piece P = eval_interval(recref(t), recref((t + 1) & (kThreads - 1)), kTwoPi / double(kThreads));
       dA[t] = P.dA;
       er[t] = P.err;

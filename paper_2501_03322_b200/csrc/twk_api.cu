@@ -16,6 +16,7 @@ constexpr int kStage2Cap = 512;         // sample capacity of refinement stage 2
 constexpr int kStage2CtasPerSM = 6;
 constexpr int kStage3CtasPerSM = 2;
 constexpr int kFixedTile = 128;
+constexpr size_t kDefaultHandoffSlots = size_t(1) << 19;   // 524,288 slots x 14,592 B = 7.6 GB
 
 thread_local char g_cuda_msg[256] = "";
 
@@ -39,17 +40,25 @@ Plan make_plan(const twk_options& o, int sms) {
 
 size_t align256(size_t x) { return (x + 255) & ~size_t(255); }
 
+size_t handoff_slots(const twk_options& o, size_t max_sources) {
+  if (o.max_samples < 2 * twk::kThreads) return 0;   // no refinement stage
+  const size_t want = o.handoff_slots < 0 ? kDefaultHandoffSlots : (size_t)o.handoff_slots;
+  return want < max_sources ? want : max_sources;
+}
+
 struct Layout {
-  size_t counters, pending, list1, list2, arena, total;
+  size_t counters, list1, list2, handoff, arena, total;
+  size_t slots;
 };
 Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
   const Plan P = make_plan(o, sms);
   Layout L{};
   size_t off = 0;
+  L.slots = handoff_slots(o, max_sources);
   L.counters = off; off += 256;
-  L.pending = off;  off += align256(max_sources);
   L.list1 = off;    off += align256(max_sources * 4);
   L.list2 = off;    off += align256(max_sources * 4);
+  L.handoff = off;  off += align256(L.slots * twk::kHandDoubles * 8);
   L.arena = off;    off += align256(P.arena_doubles * 8);
   L.total = off;
   return L;
@@ -57,7 +66,7 @@ Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
 
 bool valid_options(const twk_options& o) {
   return o.samples_per_iter == twk::kThreads && o.initial_samples == twk::kThreads && o.max_samples >= twk::kThreads &&
-         o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1);
+         o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1) && o.handoff_slots >= -1;
 }
 
 int cuda_fail(cudaError_t e) {
@@ -84,7 +93,7 @@ struct twk_ctx {
   size_t stage_bytes;
   int last_launches;
   int timing;            // record CUDA events around every stage (twk_enable_stage_timing)
-  cudaEvent_t ev[5];     // start, after stage 1, after compaction, after stage 2, after stage 3
+  cudaEvent_t ev[5];     // start, after stage 1, after stage 2, after stage 3
   int ev_used;           // number of events recorded by the last call
 };
 
@@ -96,6 +105,7 @@ void twk_default_options(twk_options* opt) {
   opt->initial_samples = 64;
   opt->max_samples = 4096;
   opt->subtract_avg_tol = 1;
+  opt->handoff_slots = -1;
 }
 
 size_t twk_workspace_bytes(const twk_options* opt, size_t max_sources) {
@@ -190,7 +200,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
   a.out_nsamples = out_nsamples;
   a.out_status = out_status;
   a.arena = reinterpret_cast<double*>(ctx->ws + ctx->lay.arena);
-  uint8_t* pending = reinterpret_cast<uint8_t*>(ctx->ws + ctx->lay.pending);
+  double* handoff = reinterpret_cast<double*>(ctx->ws + ctx->lay.handoff);
   int32_t* list1 = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list1);
   int32_t* list2 = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list2);
   int launches = 0;
@@ -206,7 +216,10 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     a1.tol = rel_tol;
     a1.final_stage = P.cap2 ? 0 : 1;
     a1.cursor = counters + 0;
-    a1.pending = pending;
+    a1.list = list1;
+    a1.list_count = counters + 1;
+    a1.handoff = handoff;
+    a1.handoff_slots = (long long)ctx->lay.slots;
     a1.out_mu = out_mu;
     a1.out_err = out_err;
     a1.out_nsamples = out_nsamples;
@@ -219,13 +232,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     mark();
   }
   if (P.cap2) {
-    // ---- a9: compact the unfinished sources (ballot + prefix sum) ---------------------------------------------------
-    const long long blocks = ((long long)n_sources + 255) / 256;
-    const int grid = (int)(blocks < 4096 ? blocks : 4096);
-    twk::compact_kernel<<<grid, 256, 0, stream>>>(pending, (long long)n_sources, list1, counters + 1);
-    ++launches;
-    mark();
-    // ---- stage 2 -----------------------------------------------------------------------------------------------------
+    // ---- stage 2: the worklist stage 1 appended (a9), first iteration handed over -------------------------------------
     twk::AdaptArgs a2 = a;
     a2.cap = P.cap2;
     a2.final_stage = P.cap3 ? 0 : 1;
@@ -234,6 +241,8 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     a2.cursor = counters + 2;
     a2.next_list = list2;
     a2.next_count = counters + 3;
+    a2.handoff = handoff;
+    a2.handoff_slots = (long long)ctx->lay.slots;
     twk::adaptive_kernel<<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2), stream>>>(a2);
     ++launches;
     mark();
@@ -341,12 +350,12 @@ int twk_enable_stage_timing(twk_ctx* ctx, int on) {
   return TWK_OK;
 }
 
-int twk_last_stage_ms(twk_ctx* ctx, float* ms4) {
-  if (!ctx || !ms4) return TWK_EINVAL;
-  for (int i = 0; i < 4; ++i) ms4[i] = 0.0f;
+int twk_last_stage_ms(twk_ctx* ctx, float* ms3) {
+  if (!ctx || !ms3) return TWK_EINVAL;
+  for (int i = 0; i < 3; ++i) ms3[i] = 0.0f;
   if (!ctx->timing || ctx->ev_used < 2) return TWK_EINVAL;
   TWK_CUDA(cudaEventSynchronize(ctx->ev[ctx->ev_used - 1]));
-  for (int i = 0; i + 1 < ctx->ev_used; ++i) TWK_CUDA(cudaEventElapsedTime(&ms4[i], ctx->ev[i], ctx->ev[i + 1]));
+  for (int i = 0; i + 1 < ctx->ev_used && i < 3; ++i) TWK_CUDA(cudaEventElapsedTime(&ms3[i], ctx->ev[i], ctx->ev[i + 1]));
   return TWK_OK;
 }
 

@@ -13,7 +13,7 @@ namespace twk {
 //   [10..14] Re z'    z' = dz/dtheta, Eq.(10) (conj on f' restored)
 //   [15..19] Im z'
 //   [20..24] z'^z''   Eq.(10) (division by J restored)
-//   [25]    nreal (3 or 5) + 8 * repaired, stored as a double
+//   [25]    nreal (3 or 5) + 8 * repaired + 16 * non-finite, stored as a double
 // In shared memory the record is a column of a [26][TILE] array (stride = TILE, conflict-free); in the global
 // arena it is 26 contiguous doubles (stride = 1, 208 B).
 // ------------------------------------------------------------------------------------------------------------
@@ -28,7 +28,7 @@ struct RecRef {
   TWK_HD cd zp(int slot) const { return mk(base[(kPX + slot) * stride], base[(kPY + slot) * stride]); }
   TWK_HD double w(int slot) const { return base[(kW + slot) * stride]; }
   TWK_HD int nreal() const { return int(base[kNR * stride]) & 7; }
-  TWK_HD int repaired() const { return int(base[kNR * stride]) >> 3; }
+  TWK_HD int point_flags() const { return int(base[kNR * stride]) >> 3; }   // kPointRepaired | kPointNonFinite
 };
 
 constexpr int kPointRepaired = 1;   // parity sum was not -1 and was repaired (G-5)
@@ -38,9 +38,10 @@ constexpr int kPointNonFinite = 2;  // a root or a derived quantity is not finit
 // a1 + a2 + a3 + a4 + a5: one boundary point source.
 // Writes the record; optionally the five roots (CM frame), their kinds and the real-image count.
 // ------------------------------------------------------------------------------------------------------------
-// cs, sn = cos(theta), sin(theta).  seeds: nullptr = cold solve; otherwise five planet-frame roots of a nearby point
-// source (element k at seeds[k * seed_stride] (re) and seeds[(5 + k) * seed_stride] (im)) for the seeded Newton
-// solve, with the cold solver as verified fallback.
+// cs, sn = cos(theta), sin(theta).  seeds: nullptr = cold solve; otherwise the source's seed block written by
+// centre_seeds() (element e at seeds[e * seed_stride]): every root of the boundary sample is predicted to first order
+// from the centre's root, eta_k + A_k delta + B_k conj(delta) with delta = rho e^{i theta}, and refined by the seeded
+// Newton solve, with the cold solver as verified fallback.
 TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn, const double* seeds, int seed_stride,
                           RecRef rec, double* out_z, int8_t* out_kind, int8_t* out_count) {
   const cd zeta = mk(fma(rho, cs, zc.x), fma(rho, sn, zc.y));
@@ -50,11 +51,21 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   coeffs_eq6(y, L.s, L.m2, c);
   bool solved = false;
   if (seeds) {
+    const double dx = rho * cs, dy = rho * sn;                  // delta
 #pragma unroll
-    for (int k = 0; k < 5; ++k) eta[k] = mk(seeds[k * seed_stride], seeds[(5 + k) * seed_stride]);
+    for (int k = 0; k < 5; ++k) {
+      const double ex = seeds[k * seed_stride], ey = seeds[(5 + k) * seed_stride];
+      const double ax = seeds[(10 + k) * seed_stride], ay = seeds[(15 + k) * seed_stride];
+      const double bx = seeds[(20 + k) * seed_stride], by = seeds[(25 + k) * seed_stride];
+      // A delta + B conj(delta)
+      eta[k] = mk(ex + fma(ax + bx, dx, (by - ay) * dy), ey + fma(ay + by, dx, (ax - bx) * dy));
+    }
     solved = quintic_roots_seeded(c, eta);
   }
-  if (!solved) quintic_roots(c, eta);
+  if (!solved) {
+    TWK_COUNT(cold_solve);
+    quintic_roots(c, eta);
+  }
 
   // a4: f', f'', residual, Jacobian in the planet frame (z2 - z = -eta, z1 - z = -s - eta; both are frame
   // invariant)
@@ -140,7 +151,7 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
       rec.at(kW + slot) = w;
     }
   }
-  rec.at(kNR) = double(nreal + ((flags & kPointRepaired) ? 8 : 0));
+  rec.at(kNR) = double(nreal + 8 * flags);
   if (out_count) *out_count = (int8_t)nreal;
   return flags;
 }
@@ -152,11 +163,53 @@ TWK_HD int point_solve(const Lens& L, cd zc, double rho, double theta, RecRef re
   return point_solve_cs(L, zc, rho, cs, sn, nullptr, 0, rec, out_z, out_kind, out_count);
 }
 
-// Cold solve of the point source at the source CENTRE: its five planet-frame roots seed the boundary samples.
-TWK_HD void centre_roots(const Lens& L, cd zc, cd (&eta)[5]) {
-  cd c[6];
-  coeffs_eq6(mk(zc.x - L.z2, zc.y), L.s, L.m2, c);
+// Seed block of one source (kSeedDoubles doubles, element e at seeds[e * stride]):
+//   [0..4] Re eta_k, [5..9] Im eta_k   the five planet-frame roots of the point source at the source CENTRE (cold solve)
+//   [10..14] Re A_k, [15..19] Im A_k, [20..24] Re B_k, [25..29] Im B_k
+//                                      first-order response of root k to a displacement delta of the source:
+//                                      d eta_k = A_k delta + B_k conj(delta)
+// The quintic's roots are the fixed points (real images) and the 2-cycle (ghost pair) of T(z) = zeta - conj f(z)
+// (G-1): z_a = zeta - conj f(z_b), z_b = zeta - conj f(z_a), with z_b = z_a for a real image.
+// Differentiating both and eliminating dz_b gives dz_a (1 - f'(w_a) f'(z_a)) = delta - f'(w_a) conj(delta) with
+// w_a = conj(z_b) = conj(zeta) - f(z_a); conj(f'(z_b)) = f'(conj z_b) because both lenses are on the real axis.  For
+// a real image this is Eq.(10)'s z'.  A prediction is kept only when the shift rho (|A| + |B|) stays below
+// a quarter of the distance to the nearest other root (next to a caustic 1/J blows up); otherwise A = B = 0.
+constexpr int kSeedDoubles = 30;
+
+TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int stride) {
+  cd c[6], eta[5];
+  const cd y = mk(zc.x - L.z2, zc.y);
+  coeffs_eq6(y, L.s, L.m2, c);
   quintic_roots(c, eta);
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const cd a = crecip(mk(-L.s - eta[k].x, -eta[k].y));
+    const cd b = crecip(-eta[k]);
+    const cd f = L.m1 * a + L.m2 * b;
+    const cd fz = L.m1 * (a * a) + L.m2 * (b * b);
+    const cd w = mk(y.x - f.x, -y.y - f.y);                    // conj(eta_b) = conj(y) - f(z_a), planet frame
+    const cd aw = crecip(mk(-L.s - w.x, -w.y));
+    const cd bw = crecip(-w);
+    const cd fw = L.m1 * (aw * aw) + L.m2 * (bw * bw);
+    const cd den = mk(1.0, 0.0) - fw * fz;
+    cd A = crecip(den);
+    cd B = -(fw * A);
+    double dmin2 = 1e300;
+#pragma unroll
+    for (int j = 0; j < 5; ++j)
+      if (j != k) dmin2 = fmin(dmin2, norm2(eta[k] - eta[j]));
+    const double shift = rho * (sqrt(norm2(A)) + sqrt(norm2(B)));
+    if (!(shift * shift <= 0.0625 * dmin2)) {                   // also catches NaN / inf
+      A = mk(0.0, 0.0);
+      B = mk(0.0, 0.0);
+    }
+    seeds[k * stride] = eta[k].x;
+    seeds[(5 + k) * stride] = eta[k].y;
+    seeds[(10 + k) * stride] = A.x;
+    seeds[(15 + k) * stride] = A.y;
+    seeds[(20 + k) * stride] = B.x;
+    seeds[(25 + k) * stride] = B.y;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------------------

@@ -21,6 +21,9 @@
 #ifndef TWK_HD
 #define TWK_HD __device__ __forceinline__
 #endif
+#ifndef TWK_COUNT
+#define TWK_COUNT(what)   // event counter hook of the host-side probes; nothing in the library
+#endif
 
 namespace twk {
 
@@ -223,36 +226,48 @@ TWK_HD void quintic_roots(const cd (&c)[6], cd (&r)[5]) {
 }
 
 // Seeded solve: Newton iteration on the ORIGINAL quintic for all five roots at once (five independent chains),
-// started from the roots of a nearby point source (the source centre, or the neighbouring boundary sample).
-// Roots of a polynomial are continuous in its coefficients, so ghosts can be followed like real images.
+// started from predictions of the roots (centre_seeds() in twk_contour.cuh).  Roots of a polynomial are continuous
+// in its coefficients, so ghosts can be followed like real images.
+// Stop rule per root: Newton converges quadratically, |dx_{n+1}| ~ K |dx_n|^2 with K ~ |dx_n| / |dx_{n-1}|^2, so
+// the step AFTER the one just taken would be ~ |dx_n|^3 / |dx_{n-1}|^2; once that is below eps/8 |r| the root is
+// converged and the confirming evaluation is skipped.  From the third iteration on the residual is also compared
+// with the rounding floor of its own evaluation (ill-conditioned roots next to a caustic stall there).
 // Returns true when every root converged and the five are distinct (Vieta: sum of roots = -c4/c5); otherwise the
 // caller falls back to the cold solver quintic_roots().  r[] holds the seeds on entry and the roots on exit.
 TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5]) {
-  double c1[6];
+  double prev[5];
 #pragma unroll
-  for (int i = 0; i < 6; ++i) c1[i] = abs1(c[i]);
+  for (int k = 0; k < 5; ++k) prev[k] = 0.0;
   unsigned done = 0;
-  for (int it = 0; it < 10 && done != 31u; ++it) {
+  for (int it = 0; it < 12 && done != 31u; ++it) {
+    const bool floor_check = it >= 2;
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
+      if (done & (1u << k)) continue;
+      TWK_COUNT(newton_eval);
       cd p = c[5], d = mk(0.0, 0.0);
-      double err = c1[5];
-      const double ax = abs1(r[k]);
 #pragma unroll
       for (int i = 4; i >= 0; --i) {
         d = cfma(d, r[k], p);
         p = cfma(p, r[k], c[i]);
-        err = fma(err, ax, c1[i]);
       }
-      if (abs1(p) <= 2.0 * kEps * err) { done |= 1u << k; continue; }   // at the rounding floor
+      if (floor_check) {
+        const double ax = abs1(r[k]);
+        double err = abs1(c[5]);
+#pragma unroll
+        for (int i = 4; i >= 0; --i) err = fma(err, ax, abs1(c[i]));
+        if (abs1(p) <= 2.0 * kEps * err) { done |= 1u << k; continue; }   // at the rounding floor
+      }
       const double dn = norm2(d);
       if (!(dn > 0.0)) continue;
       const cd dx = cdiv(p, d);
       r[k] = r[k] - dx;
-      if (abs1(dx) <= 1e-12 * abs1(r[k])) done |= 1u << k;
+      const double sdx = abs1(dx), ar = abs1(r[k]);
+      if (sdx * sdx * sdx <= (0.125 * kEps) * ar * prev[k] * prev[k] || sdx <= kEps * ar) done |= 1u << k;
+      prev[k] = sdx;
     }
   }
-  if (done != 31u) return false;
+  if (done != 31u) { TWK_COUNT(fail_iter); return false; }
   // distinctness: sum of the roots against -c4/c5
   const cd want = -cdiv(c[4], c[5]);
   const cd sum = (r[0] + r[1]) + (r[2] + r[3]) + r[4];

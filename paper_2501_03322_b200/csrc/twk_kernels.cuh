@@ -5,10 +5,9 @@
 //   adaptive_kernel   the adaptive loop of P:318-326 for one source per 64-thread CTA, entirely on-device:
 //                     64 samples per iteration (one thread each), per-source sorted sample state in shared memory,
 //                     error-weighted inverse-transform sampling, stop rule + cap.
-//                     Stage 1 (kStage1): cap = 64, records in shared memory, every source of the batch;
-//                     stages 2/3: larger caps, records in a per-CTA global arena (L2 resident), sources taken
-//                     from the compacted worklist of the previous stage.
-//   compact_kernel    a9: worklist of unfinished sources by warp ballot + prefix sum
+//                     Refinement stages 2/3 (twk_adaptive.cuh): records in a per-CTA global arena (L2 resident),
+//                     sources taken from the worklist of the previous stage.  Stage 1 (twk_stage1.cuh) is the
+//                     first iteration of every source, everything in shared memory.
 //   dfma_probe_kernel FP64 FMA throughput probe (roofline denominator)
 #pragma once
 
@@ -21,6 +20,8 @@ namespace twk {
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr double kPi = 3.141592653589793238462643383279;
 constexpr int kThreads = 64;   // threads per source = samples per iteration
+// Hand-over slot (stage 1 -> stage 2), in doubles: records [26][64] | dA [64] | err [64] | seed block [30] (+2 pad)
+constexpr int kHandDoubles = (kRecDoubles + 2) * kThreads + 32;
 
 struct Batch {
   const double* s;
@@ -141,36 +142,6 @@ __global__ void __launch_bounds__(TILE) fixed_kernel(Batch b, int N, double* __r
       if (out_mu) out_mu[src] = A / (kPi * S.rho * S.rho);
       if (out_err) out_err[src] = E / fabs(A);
     }
-    __syncthreads();
-  }
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// a9. worklist compaction: ids of sources with pending[i] != 0, by warp ballot + prefix sum.
-// ------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) compact_kernel(const uint8_t* __restrict__ pending, long long n, int32_t* __restrict__ list,
-                                                      int* __restrict__ count) {
-  __shared__ int warp_tot[8];
-  __shared__ int block_base;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (long long base = (long long)blockIdx.x * 256; base < n; base += (long long)gridDim.x * 256) {
-    const long long i = base + threadIdx.x;
-    const bool p = (i < n) && pending[i];
-    const unsigned bal = __ballot_sync(0xffffffffu, p);
-    const int within = __popc(bal & ((1u << lane) - 1u));
-    if (lane == 0) warp_tot[warp] = __popc(bal);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      int tot = 0;
-      for (int w = 0; w < 8; ++w) {
-        const int c = warp_tot[w];
-        warp_tot[w] = tot;
-        tot += c;
-      }
-      block_base = tot ? atomicAdd(count, tot) : 0;
-    }
-    __syncthreads();
-    if (p) list[block_base + warp_tot[warp] + within] = (int32_t)i;
     __syncthreads();
   }
 }

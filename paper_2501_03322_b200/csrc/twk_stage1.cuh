@@ -2,12 +2,15 @@
 //
 // One 64-thread CTA takes a group of 64 consecutive sources from an atomic cursor:
 //   phase 1  thread i cold-solves the point source at the CENTRE of source i (Laguerre + deflation): its five
-//            planet-frame roots are the seeds of that source's boundary samples (roots are continuous in zeta);
+//            planet-frame roots and their first-order response to a source displacement are the seeds of that
+//            source's boundary samples (centre_seeds(), twk_contour.cuh);
 //   phase 2  for each source of the group: thread t solves boundary sample t by seeded Newton on the undeflated
 //            quintic (verified; cold fallback), writes its record to shared memory, evaluates interval (t, t+1),
-//            block-reduces area and error and applies the stop rule;
-//   phase 3  coalesced write of the group's results; unfinished sources are flagged in `pending` (-> stage 2).
-// Per-source state never leaves the SM: records [26][64], seeds [10][64], parameters [8][64], results.
+//            block-reduces area and error and applies the stop rule.  An unfinished source is appended to
+//            the refinement worklist (a9) and its whole first-iteration state -- 64 records, 64 interval
+//            pieces, seeds -- is handed to stage 2 through the hand-over arena (coalesced 512 B rows);
+//   phase 3  coalesced write of the group's results.
+// Per-source state of a finished source never leaves the SM: records [26][64], seeds [30][64], parameters [8][64].
 #pragma once
 
 #include "twk_kernels.cuh"
@@ -19,7 +22,10 @@ struct Stage1Args {
   double tol;
   int final_stage;       // 1: there is no refinement stage (max_samples < 128): cap status instead of pending
   int* cursor;           // group fetch counter (zeroed before launch)
-  uint8_t* pending;      // [n_sources] 1 = needs refinement
+  int32_t* list;         // [n_sources] a9: worklist of unfinished sources, appended in completion order
+  int* list_count;       // entries of `list` (zeroed before launch)
+  double* handoff;       // [handoff_slots][kHandDoubles] first-iteration state of worklist entries < handoff_slots
+  long long handoff_slots;
   double* out_mu;
   double* out_err;       // may be null
   int32_t* out_nsamples; // may be null
@@ -28,7 +34,7 @@ struct Stage1Args {
 
 constexpr int kS1ParamRows = 8;   // s, m1, m2, z2, Re zc, Im zc, rho, status|valid
 __host__ __device__ inline size_t stage1_smem_bytes() {
-  return (size_t)(kRecDoubles * kThreads + 10 * kThreads + kS1ParamRows * kThreads + 2 * kThreads + 8) * 8 +
+  return (size_t)(kRecDoubles * kThreads + kSeedDoubles * kThreads + kS1ParamRows * kThreads + 2 * kThreads + 8) * 8 +
          (size_t)(2 * kThreads + 4) * 4 + kThreads;
 }
 
@@ -57,8 +63,8 @@ __device__ __forceinline__ void block_sum2_or(double& a, double& b, int& f, doub
 __global__ void __launch_bounds__(kThreads, 6) stage1_kernel(Stage1Args p) {
   extern __shared__ double sm[];
   double* recs = sm;                                   // [26][64]
-  double* seeds = recs + kRecDoubles * kThreads;       // [10][64]: rows 0-4 Re eta_k, rows 5-9 Im eta_k; column = source
-  double* prm = seeds + 10 * kThreads;                 // [8][64]
+  double* seeds = recs + kRecDoubles * kThreads;       // [30][64]: seed block (twk_contour.cuh); column = source
+  double* prm = seeds + kSeedDoubles * kThreads;       // [8][64]
   double* res_mu = prm + kS1ParamRows * kThreads;      // [64]
   double* res_err = res_mu + kThreads;                 // [64]
   double* scratch = res_err + kThreads;                // [8]
@@ -95,15 +101,7 @@ __global__ void __launch_bounds__(kThreads, 6) stage1_kernel(Stage1Args p) {
         prm[5 * kThreads + t] = S.zc.y;
         prm[6 * kThreads + t] = S.rho;
         prm[7 * kThreads + t] = double((int)S.status | (S.valid ? 256 : 0));
-        if (S.valid) {
-          cd eta[5];
-          centre_roots(S.L, S.zc, eta);
-#pragma unroll
-          for (int k = 0; k < 5; ++k) {
-            seeds[k * kThreads + t] = eta[k].x;
-            seeds[(5 + k) * kThreads + t] = eta[k].y;
-          }
-        }
+        if (S.valid) centre_seeds(S.L, S.zc, S.rho, seeds + t, kThreads);
       }
     }
     __syncthreads();
@@ -133,13 +131,32 @@ __global__ void __launch_bounds__(kThreads, 6) stage1_kernel(Stage1Args p) {
       const Piece P = eval_interval(mine, next, kTwoPi / double(kThreads));
       double A = P.dA, E = P.err;
       block_sum2_or(A, E, flags, scratch, iscr + 1);
+      // every thread holds A, E: the decision is uniform
+      const bool finite = isfinite(A) && isfinite(E);
+      const bool pend = finite && !(E <= p.tol * fabs(A)) && !p.final_stage;   // stop rule P:272
+      if (pend) {
+        // a9: append to the refinement worklist; hand the first-iteration state over when a slot is free
+        if (t == 0) {
+          const int slot = atomicAdd(p.list_count, 1);
+          p.list[slot] = (int32_t)(base + i);
+          iscr[3] = slot;
+        }
+        __syncthreads();
+        const long long slot = iscr[3];
+        if (slot < p.handoff_slots) {
+          double* h = p.handoff + (size_t)slot * kHandDoubles;
+#pragma unroll
+          for (int e = 0; e < kRecDoubles; ++e) h[e * kThreads + t] = mine.at(e);
+          h[kRecDoubles * kThreads + t] = P.dA;
+          h[(kRecDoubles + 1) * kThreads + t] = P.err;
+          if (t < kSeedDoubles) h[(kRecDoubles + 2) * kThreads + t] = seeds[t * kThreads + i];
+        }
+      }
       if (t == 0) {
         uint32_t status = (uint32_t)(code & 255);
-        bool pend = false;
-        if (!(isfinite(A) && isfinite(E))) status |= 16u;
+        if (!finite) status |= 16u;
         else if (E <= p.tol * fabs(A)) status |= 1u;               // stop rule P:272
         else if (p.final_stage) status |= 2u;                       // cap P:326
-        else pend = true;
         if (flags & kPointRepaired) status |= 4u;
         if (flags & kPointNonFinite) status |= 16u;
         res_mu[i] = A / (kPi * rho * rho);
@@ -154,9 +171,7 @@ __global__ void __launch_bounds__(kThreads, 6) stage1_kernel(Stage1Args p) {
     {
       const long long src = base + t;
       if (src < n) {
-        const bool pend = res_pend[t] != 0;
-        p.pending[src] = pend ? 1 : 0;
-        if (!pend) {
+        if (!res_pend[t]) {
           p.out_mu[src] = res_mu[t];
           if (p.out_err) p.out_err[src] = res_err[t];
           if (p.out_nsamples) p.out_nsamples[src] = res_ns[t];

@@ -156,6 +156,27 @@ def test_full_size_config3_sampled_outputs(ctx):
     assert np.median(rel) < 1e-5
 
 
+def test_handover_and_recompute_paths_agree():
+    """Stage 1 hands the first iteration of an unfinished source to stage 2 through the hand-over arena; without a
+    free slot stage 2 recomputes it.  Same arithmetic either way: identical sample counts and status, mu to rounding."""
+    import paper_2501_03322_b200 as P
+    full = W.config4()
+    zc = full.zeta[:, 0] + 1j * full.zeta[:, 1]
+    band = np.where((np.abs(zc.imag) < 0.25) & (np.abs(zc.real) < 0.6))[0]
+    wl = full.subset(band[:: max(1, len(band) // 3000)])
+    res = []
+    for slots in (-1, 0, 37):
+        c = P.Context(wl.n_sources, handoff_slots=slots)
+        res.append(c.magnify_workload(wl, 1e-5))
+        st = c.twk_last_stats()
+        assert st["n_stage2"] > 1000           # most of the band refines
+        c.close()
+    for r in res[1:]:
+        assert np.array_equal(r["nsamples"], res[0]["nsamples"])
+        assert np.array_equal(r["status"], res[0]["status"])
+        assert np.abs(r["mu"] / res[0]["mu"] - 1).max() < 1e-12
+
+
 def test_edge_cases(ctx):
     import torch
     import paper_2501_03322_b200 as P
