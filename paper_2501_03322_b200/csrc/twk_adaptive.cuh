@@ -80,130 +80,130 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
     }
     // ---- first iteration: 64 uniform samples theta_j = 2 pi j / 64 (reading A-3) ----------------------
     int flags = 0;
-    theta[t] = kTwoPi * double(t) / double(kThreads);
-    ids[t] = (uint16_t)t;
+    int n = 0;
     hand = (p.handoff && cur < p.handoff_slots) ? p.handoff + (size_t)cur * kHandDoubles : nullptr;
     if (hand) {   // done by stage 1: take its interval pieces and seed block, use its records in place
+      theta[t] = kTwoPi * double(t) / double(kThreads);
+      ids[t] = (uint16_t)t;
       dA[t] = hand[kRecDoubles * kThreads + t];
       er[t] = hand[(kRecDoubles + 1) * kThreads + t];
       if (t < kSeedDoubles) seeds[t] = hand[(kRecDoubles + 2) * kThreads + t];
       flags |= recref(t).point_flags();
-    } else {
+      n = kThreads;
+    } else {      // not handed over: the loop below starts by inserting the 64 uniform samples into the empty list
       if (t == 0) centre_seeds(S.L, S.zc, S.rho, seeds, 1);
-      __syncthreads();
-      double sn, cs;
-      sincospi(double(t) / 32.0, &sn, &cs);
-      flags |= point_solve_cs(S.L, S.zc, S.rho, cs, sn, seeds, 1, recref(t), nullptr, nullptr, nullptr);
-      __syncthreads();
-      const Piece P = eval_interval(recref(t), recref((t + 1) & (kThreads - 1)), kTwoPi / double(kThreads));
-      dA[t] = P.dA;
-      er[t] = P.err;
     }
-    int n = kThreads;
     uint32_t status = S.status;
     bool exhausted = false;
     double A = 0.0, E = 0.0;
     for (;;) {
       __syncthreads();
-      // ---- area and error sums over all intervals (a7 reduction) ----------------------------------------------
-      double a = 0.0, e = 0.0;
-      for (int i = t; i < n; i += kThreads) {
-        a += dA[i];
-        e += er[i];
-      }
-      block_sum2(a, e, scratch);
-      A = a;
-      E = e;
-      const double tolA = p.tol * fabs(A);
-      if (!(isfinite(A) && isfinite(E))) { status |= 16u; break; }
-      if (E <= tolA) { status |= 1u; break; }                       // stop rule P:272, reading A-1
-      if (n + kThreads > cap) { exhausted = true; break; }          // cap P:326, reading A-6
-      // ---- a8: error-weighted inverse-transform sampling, 64 quantiles ---------------------------
-      const double avg = p.subtract_avg_tol ? tolA / double(n) : 0.0;   // "average tolerance", reading A-5
-      double W = 0.0, unused = 0.0;
-      for (int i = t; i < n; i += kThreads) W += fmax(er[i] - avg, 0.0);
-      block_sum2(W, unused, scratch);
-      const bool raw = !(W > 0.0);
-      if (raw) W = E;
-      const double scale = double(kThreads) / W;
-      newint[t] = -1;
-      double carry = 0.0;
-      for (int base = 0; base < n; base += kThreads) {
-        const int i = base + t;
-        const double w = (i < n) ? (raw ? er[i] : fmax(er[i] - avg, 0.0)) : 0.0;
-        double x = w;   // inclusive scan over the 64 threads
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const double y = __shfl_up_sync(0xffffffffu, x, o);
-          if (lane >= o) x += y;
+      int m = kThreads;
+      if (n == 0) {
+        cth[t] = kTwoPi * double(t) / double(kThreads);
+        cint[t] = -1;
+        __syncthreads();
+      } else {
+        // ---- area and error sums over all intervals (a7 reduction) ----------------------------------------------
+        double a = 0.0, e = 0.0;
+        for (int i = t; i < n; i += kThreads) {
+          a += dA[i];
+          e += er[i];
         }
-        __syncthreads();
-        if (lane == 31) scratch[4 + warp] = x;
-        __syncthreads();
-        const double w0 = scratch[4], w1 = scratch[5];
-        if (warp == 1) x += w0;
-        const double cum_incl = carry + x;
-        double cum_excl = __shfl_up_sync(0xffffffffu, cum_incl, 1);
-        if (lane == 0) cum_excl = (warp == 0) ? carry : carry + w0;   // bitwise the left neighbour's cum_incl
-        if (w > 0.0) {
-          // quantile k has target (k + 1/2)/64 * W (reading A-4); this interval owns those in [cum_excl, cum_incl)
-          const int klo = min(kThreads, max(0, (int)ceil(cum_excl * scale - 0.5)));
-          const int khi = min(kThreads, max(0, (int)ceil(cum_incl * scale - 0.5)));
-          const double th0 = theta[i];
-          const double hi = (i + 1 < n) ? theta[i + 1] : kTwoPi;
-          for (int k = klo; k < khi; ++k) {
-            const double target = (double(k) + 0.5) / double(kThreads) * W;
-            const double frac = (target - cum_excl) / w;
-            const double th = fma(frac, hi - th0, th0);              // linear interpolation
-            newth[k] = (th > th0 && th < hi) ? th : nan("");
-            newint[k] = i;
+        block_sum2(a, e, scratch);
+        A = a;
+        E = e;
+        const double tolA = p.tol * fabs(A);
+        if (!(isfinite(A) && isfinite(E))) { status |= 16u; break; }
+        if (E <= tolA) { status |= 1u; break; }                       // stop rule P:272, reading A-1
+        if (n + kThreads > cap) { exhausted = true; break; }          // cap P:326, reading A-6
+        // ---- a8: error-weighted inverse-transform sampling, 64 quantiles ---------------------------
+        const double avg = p.subtract_avg_tol ? tolA / double(n) : 0.0;   // "average tolerance", reading A-5
+        double W = 0.0, unused = 0.0;
+        for (int i = t; i < n; i += kThreads) W += fmax(er[i] - avg, 0.0);
+        block_sum2(W, unused, scratch);
+        const bool raw = !(W > 0.0);
+        if (raw) W = E;
+        const double scale = double(kThreads) / W;
+        newint[t] = -1;
+        double carry = 0.0;
+        for (int base = 0; base < n; base += kThreads) {
+          const int i = base + t;
+          const double w = (i < n) ? (raw ? er[i] : fmax(er[i] - avg, 0.0)) : 0.0;
+          double x = w;   // inclusive scan over the 64 threads
+  #pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            const double y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
           }
-        }
-        carry += w0 + w1;
-      }
-      __syncthreads();
-      // ---- drop invalid / duplicate angles, compact (ballot + prefix sum) --------------------------------------
-      bool v = (newint[t] >= 0) && (newth[t] == newth[t]);
-      if (v && t > 0 && newint[t - 1] == newint[t] && !(newth[t] > newth[t - 1])) v = false;
-      const unsigned bal = __ballot_sync(0xffffffffu, v);
-      if (lane == 0) iscr[1 + warp] = __popc(bal);
-      __syncthreads();
-      const int m = iscr[1] + iscr[2];
-      const int rank = __popc(bal & ((1u << lane) - 1u)) + (warp ? iscr[1] : 0);
-      if (v) {
-        cth[rank] = newth[t];
-        cint[rank] = newint[t];
-      }
-      __syncthreads();
-      if (m == 0) { exhausted = true; break; }
-      // ---- merge: old element j moves up by the number of new samples inserted before it ------------------------
-      for (int base = ((n - 1) / kThreads) * kThreads; base >= 0; base -= kThreads) {
-        const int j = base + t;
-        const bool have = j < n;
-        double v0 = 0.0, v1 = 0.0, v2 = 0.0;
-        uint16_t v3 = 0;
-        int cnt = 0;
-        if (have) {
-          v0 = theta[j];
-          v1 = dA[j];
-          v2 = er[j];
-          v3 = ids[j];
-          int lo = 0, hiq = m;   // cnt = #{r : cint[r] < j}
-          while (lo < hiq) {
-            const int mid = (lo + hiq) >> 1;
-            if (cint[mid] < j) lo = mid + 1; else hiq = mid;
+          __syncthreads();
+          if (lane == 31) scratch[4 + warp] = x;
+          __syncthreads();
+          const double w0 = scratch[4], w1 = scratch[5];
+          if (warp == 1) x += w0;
+          const double cum_incl = carry + x;
+          double cum_excl = __shfl_up_sync(0xffffffffu, cum_incl, 1);
+          if (lane == 0) cum_excl = (warp == 0) ? carry : carry + w0;   // bitwise the left neighbour's cum_incl
+          if (w > 0.0) {
+            // quantile k has target (k + 1/2)/64 * W (reading A-4); this interval owns those in [cum_excl, cum_incl)
+            const int klo = min(kThreads, max(0, (int)ceil(cum_excl * scale - 0.5)));
+            const int khi = min(kThreads, max(0, (int)ceil(cum_incl * scale - 0.5)));
+            const double th0 = theta[i];
+            const double hi = (i + 1 < n) ? theta[i + 1] : kTwoPi;
+            for (int k = klo; k < khi; ++k) {
+              const double target = (double(k) + 0.5) / double(kThreads) * W;
+              const double frac = (target - cum_excl) / w;
+              const double th = fma(frac, hi - th0, th0);              // linear interpolation
+              newth[k] = (th > th0 && th < hi) ? th : nan("");
+              newint[k] = i;
+            }
           }
-          cnt = lo;
+          carry += w0 + w1;
         }
         __syncthreads();
-        if (have) {
-          theta[j + cnt] = v0;
-          dA[j + cnt] = v1;
-          er[j + cnt] = v2;
-          ids[j + cnt] = v3;
+        // ---- drop invalid / duplicate angles, compact (ballot + prefix sum) --------------------------------------
+        bool v = (newint[t] >= 0) && (newth[t] == newth[t]);
+        if (v && t > 0 && newint[t - 1] == newint[t] && !(newth[t] > newth[t - 1])) v = false;
+        const unsigned bal = __ballot_sync(0xffffffffu, v);
+        if (lane == 0) iscr[1 + warp] = __popc(bal);
+        __syncthreads();
+        m = iscr[1] + iscr[2];
+        const int rank = __popc(bal & ((1u << lane) - 1u)) + (warp ? iscr[1] : 0);
+        if (v) {
+          cth[rank] = newth[t];
+          cint[rank] = newint[t];
         }
         __syncthreads();
-      }
+        if (m == 0) { exhausted = true; break; }
+        // ---- merge: old element j moves up by the number of new samples inserted before it ------------------------
+        for (int base = ((n - 1) / kThreads) * kThreads; base >= 0; base -= kThreads) {
+          const int j = base + t;
+          const bool have = j < n;
+          double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+          uint16_t v3 = 0;
+          int cnt = 0;
+          if (have) {
+            v0 = theta[j];
+            v1 = dA[j];
+            v2 = er[j];
+            v3 = ids[j];
+            int lo = 0, hiq = m;   // cnt = #{r : cint[r] < j}
+            while (lo < hiq) {
+              const int mid = (lo + hiq) >> 1;
+              if (cint[mid] < j) lo = mid + 1; else hiq = mid;
+            }
+            cnt = lo;
+          }
+          __syncthreads();
+          if (have) {
+            theta[j + cnt] = v0;
+            dA[j + cnt] = v1;
+            er[j + cnt] = v2;
+            ids[j + cnt] = v3;
+          }
+          __syncthreads();
+        }
+      }   // n > 0
       // ---- solve the new samples (a1-a5 only for the newly added) -----------------------------------------
       const int pos = (t < m) ? cint[t] + 1 + t : 0;
       if (t < m) {
@@ -211,25 +211,25 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         theta[pos] = th;
         ids[pos] = (uint16_t)(n + t);
         double sn, cs;
-        sincos(th, &sn, &cs);
+        if (n == 0) sincospi(double(t) / 32.0, &sn, &cs);   // exactly stage 1's angles
+        else sincos(th, &sn, &cs);
         flags |= point_solve_cs(S.L, S.zc, S.rho, cs, sn, seeds, 1, recref(n + t), nullptr, nullptr, nullptr);
       }
       const int n_new = n + m;
       __syncthreads();
-      // ---- re-evaluate only the intervals that changed ----------------------------------------------------
+      // ---- re-evaluate only the intervals that changed: the one to the left of every new sample, and the
+      //      one to its right when the next sample is old (or the list wraps around) ---------------------------------
       if (t < m) {
-        {
-          const Piece P = eval_interval(recref(ids[pos - 1]), recref(n + t), theta[pos] - theta[pos - 1]);
-          dA[pos - 1] = P.dA;
-          er[pos - 1] = P.err;
-        }
         const bool last_in_group = (t == m - 1) || (cint[t + 1] != cint[t]);
-        if (last_in_group) {
-          const int nxt = (pos + 1 < n_new) ? pos + 1 : 0;
-          const double dth = (pos + 1 < n_new) ? theta[pos + 1] - theta[pos] : kTwoPi - theta[pos];
-          const Piece P = eval_interval(recref(n + t), recref(ids[nxt]), dth);
-          dA[pos] = P.dA;
-          er[pos] = P.err;
+#pragma unroll 1
+        for (int side = 0; side < 2; ++side) {
+          if (side == 0 ? (pos == 0) : !last_in_group) continue;
+          const int ia = pos - 1 + side;                       // interval (ia, ia + 1)
+          const int ib = (ia + 1 < n_new) ? ia + 1 : 0;
+          const double dth = (ia + 1 < n_new) ? theta[ia + 1] - theta[ia] : kTwoPi - theta[ia];
+          const Piece P = eval_interval(recref(ids[ia]), recref(ids[ib]), dth);
+          dA[ia] = P.dA;
+          er[ia] = P.err;
         }
       }
       n = n_new;

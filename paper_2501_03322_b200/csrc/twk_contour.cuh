@@ -64,7 +64,12 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   }
   if (!solved) {
     TWK_COUNT(cold_solve);
-    quintic_roots(c, eta);
+    Coef6 C;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) C.c[i] = c[i];
+    const Roots5 R = quintic_roots_cold(C);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) eta[k] = R.r[k];
   }
 
   // a4: f', f'', residual, Jacobian in the planet frame (z2 - z = -eta, z1 - z = -s - eta; both are frame
@@ -180,7 +185,14 @@ TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int st
   cd c[6], eta[5];
   const cd y = mk(zc.x - L.z2, zc.y);
   coeffs_eq6(y, L.s, L.m2, c);
-  quintic_roots(c, eta);
+  {
+    Coef6 C;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) C.c[i] = c[i];
+    const Roots5 R = quintic_roots_cold(C);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) eta[k] = R.r[k];
+  }
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
     const cd a = crecip(mk(-L.s - eta[k].x, -eta[k].y));
@@ -238,6 +250,16 @@ TWK_HD void link_terms(const RecRef& A, const RecRef& B, int ka, int kb, double 
   err += (E1 + E2) + (E3 + E4);
 }
 
+// 2 x 2 minimum-total-distance matching from SQUARED distances: returns 1 when the crossed pairing (0-1, 1-0) is
+// shorter than the straight one (0-0, 1-1); ties keep the straight pairing (reading L-3).  When one pairing has
+// both distances below half of both distances of the other, 2 max < min settles the comparison of the sums without
+// square roots (the decision is the same as the exact one whenever the shortcut applies).
+TWK_HD int crossed_is_shorter(double s00, double s11, double s01, double s10) {
+  if (4.0 * fmax(s00, s11) < fmin(s01, s10)) return 0;
+  if (4.0 * fmax(s01, s10) < fmin(s00, s11)) return 1;
+  return (sqrt(s01) + sqrt(s10)) < (sqrt(s00) + sqrt(s11));
+}
+
 TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth) {
   Piece P;
   P.dA = 0.0;
@@ -245,30 +267,40 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth) {
   P.crossing = 0;
   const bool a5 = A.nreal() == 5, b5 = B.nreal() == 5;
   int leftApos = -1, leftAneg = -1, leftBpos = -1, leftBneg = -1;
+  // links are collected first (slot of A | slot of B << 4, one byte each) and evaluated in ONE loop below
+  unsigned long long links = 0;
+  int nl = 0;
+  auto add_link = [&](int ka, int kb) {
+    links |= (unsigned long long)(ka | (kb << 4)) << (8 * nl);
+    ++nl;
+  };
   // ---- positive parity: slots 0,(1) --------------------------------------------------------------------
   {
     const cd A0 = A.z(0), B0 = B.z(0);
     if (!a5 && !b5) {
-      link_terms(A, B, 0, 0, 1.0, dth, P.dA, P.err);
+      add_link(0, 0);
     } else if (a5 && b5) {
       const cd A1 = A.z(1), B1 = B.z(1);
-      const double straight = sqrt(norm2(A0 - B0)) + sqrt(norm2(A1 - B1));
-      const double crossed = sqrt(norm2(A0 - B1)) + sqrt(norm2(A1 - B0));
-      const int sw = crossed < straight;
-      link_terms(A, B, 0, sw, 1.0, dth, P.dA, P.err);
-      link_terms(A, B, 1, 1 - sw, 1.0, dth, P.dA, P.err);
+      const int sw = crossed_is_shorter(norm2(A0 - B0), norm2(A1 - B1), norm2(A0 - B1), norm2(A1 - B0));
+      add_link(0, sw);
+      add_link(1, 1 - sw);
     } else if (b5) {   // 1 -> 2: the nearer one links, the other is left over
       const int j = norm2(A0 - B.z(1)) < norm2(A0 - B0);
-      link_terms(A, B, 0, j, 1.0, dth, P.dA, P.err);
+      add_link(0, j);
       leftBpos = 1 - j;
     } else {           // 2 -> 1
       const int i = norm2(A.z(1) - B0) < norm2(A0 - B0);
-      link_terms(A, B, i, 0, 1.0, dth, P.dA, P.err);
+      add_link(i, 0);
       leftApos = 1 - i;
     }
   }
   // ---- negative parity: slots 2,3,(4): minimum-total-distance injective matching -----------------
-  {
+  if (!a5 && !b5) {
+    const cd A2 = A.z(2), A3 = A.z(3), B2 = B.z(2), B3 = B.z(3);
+    const int sw = crossed_is_shorter(norm2(A2 - B2), norm2(A3 - B3), norm2(A2 - B3), norm2(A3 - B2));
+    add_link(2, 2 + sw);
+    add_link(3, 3 - sw);
+  } else {
     const int na = a5 ? 3 : 2, nb = b5 ? 3 : 2;
     double D[3][3];
     cd za[3], zb[3];
@@ -282,9 +314,8 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth) {
 #pragma unroll
       for (int j = 0; j < 3; ++j) {
         const bool ra = i < na, rb = j < nb;
-        // a missing third image is a dummy: free against real images when only one side lacks it, and forced
-        // onto the other dummy when both sides lack it
-        D[i][j] = (ra && rb) ? sqrt(norm2(za[i] - zb[j])) : ((ra || rb) ? ((na == nb) ? 1e300 : 0.0) : 0.0);
+        // a missing third image is a dummy: free against real images (only one side lacks it here)
+        D[i][j] = (ra && rb) ? sqrt(norm2(za[i] - zb[j])) : 0.0;
       }
     const int perm[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
     int bestp = 0;
@@ -301,10 +332,17 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth) {
       for (int p = 0; p < 6; ++p)
         if (p == bestp) j = perm[p][i];
       const bool ra = i < na, rb = j < nb;
-      if (ra && rb) link_terms(A, B, 2 + i, 2 + j, -1.0, dth, P.dA, P.err);
+      if (ra && rb) add_link(2 + i, 2 + j);
       else if (ra) leftAneg = 2 + i;
       else if (rb) leftBneg = 2 + j;
     }
+  }
+  // ---- a7: area and error of every link (one copy of the code; 3 or 4 or 5 trips) ----------------------------
+#pragma unroll 1
+  for (int l = 0; l < nl; ++l) {
+    const int ka = (int)(links & 15u), kb = (int)((links >> 4) & 15u);
+    links >>= 8;
+    link_terms(A, B, ka, kb, ka < 2 ? 1.0 : -1.0, dth, P.dA, P.err);
   }
   // ---- caustic crossing: the extra (+,-) pair on the 5-image side connects to itself -------------
   if (a5 != b5) {

@@ -21,6 +21,9 @@
 #ifndef TWK_HD
 #define TWK_HD __device__ __forceinline__
 #endif
+#ifndef TWK_NOINLINE
+#define TWK_NOINLINE __device__ __noinline__   // rarely executed paths stay out of the hot instruction stream
+#endif
 #ifndef TWK_COUNT
 #define TWK_COUNT(what)   // event counter hook of the host-side probes; nothing in the library
 #endif
@@ -225,6 +228,17 @@ TWK_HD void quintic_roots(const cd (&c)[6], cd (&r)[5]) {
   }
 }
 
+// The cold solver as an out-of-line call (arguments and result by value, so the caller's coefficient and root
+// registers never have their address taken): it is the rare fallback of the seeded solve, and ~6 k instructions
+// that must not sit in the middle of the hot loop's instruction stream.
+struct Coef6 { cd c[6]; };
+struct Roots5 { cd r[5]; };
+TWK_NOINLINE Roots5 quintic_roots_cold(Coef6 C) {
+  Roots5 R;
+  quintic_roots(C.c, R.r);
+  return R;
+}
+
 // Seeded solve: Newton iteration on the ORIGINAL quintic for all five roots at once (five independent chains),
 // started from predictions of the roots (centre_seeds() in twk_contour.cuh).  Roots of a polynomial are continuous
 // in its coefficients, so ghosts can be followed like real images.
@@ -232,47 +246,136 @@ TWK_HD void quintic_roots(const cd (&c)[6], cd (&r)[5]) {
 // the step AFTER the one just taken would be ~ |dx_n|^3 / |dx_{n-1}|^2; once that is below eps/8 |r| the root is
 // converged and the confirming evaluation is skipped.  From the third iteration on the residual is also compared
 // with the rounding floor of its own evaluation (ill-conditioned roots next to a caustic stall there).
-// Returns true when every root converged and the five are distinct (Vieta: sum of roots = -c4/c5); otherwise the
-// caller falls back to the cold solver quintic_roots().  r[] holds the seeds on entry and the roots on exit.
+// Verification: all five converged and distinct (Vieta: sum of roots = -c4/c5).
+// Recovery (at most once per solve): when two chains ran into the same root, or up to two chains have not
+// converged after 10 sweeps, the three or four good distinct roots fix the others through Vieta's formulas
+// (sum of roots = -c4/c5, product = -c0/c5: one missing root directly, two as the roots of a quadratic); these
+// are polished by the same Newton sweeps and the verification is repeated.
+// Returns false when that fails too; the caller then falls back to the cold solver quintic_roots().
+// r[] holds the seeds on entry and the roots on exit.
+struct SeededState {
+  cd r[5];
+  unsigned done;
+  int ok;
+};
+// Recovery step of the seeded solve (see above), out of line.  Returns ok = 0 when fewer than three good roots are
+// left; otherwise the replaced roots are in r[] with their done bits cleared.
+TWK_NOINLINE SeededState seeded_recover(cd c0, cd c5, cd tot, SeededState S) {
+  TWK_COUNT(recovery);
+  cd (&r)[5] = S.r;
+  const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
+  // good = converged and not a duplicate of an earlier good root
+  unsigned good = S.done;
+#pragma unroll
+  for (int a = 0; a < 5; ++a)
+#pragma unroll
+    for (int b = a + 1; b < 5; ++b)
+      if ((good >> a & 1u) && (good >> b & 1u) && norm2(r[a] - r[b]) <= 1e-18 * scale * scale) good &= ~(1u << b);
+  int ng = 0;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) ng += (good >> k) & 1u;
+  S.ok = (ng == 3 || ng == 4);
+  if (!S.ok) return S;
+  cd sum = mk(0.0, 0.0), prod = mk(1.0, 0.0);
+#pragma unroll
+  for (int k = 0; k < 5; ++k)
+    if (good >> k & 1u) {
+      sum = sum + r[k];
+      prod = prod * r[k];
+    }
+  cd x1 = tot - sum, x2 = x1;
+  if (ng == 3) {   // x^2 - S x + P = 0 with S = tot - sum, P = (-c0/c5) / prod
+    const cd Ssum = x1;
+    const cd P = -cdiv(c0, c5 * prod);
+    cd sq = csqrt_(Ssum * Ssum - 4.0 * P);
+    if (dotp(Ssum, sq) < 0.0) sq = -sq;
+    x1 = 0.5 * (Ssum + sq);
+    x2 = (norm2(x1) > 0.0) ? cdiv(P, x1) : x1;
+  }
+  bool first = true;
+#pragma unroll
+  for (int k = 0; k < 5; ++k)
+    if (!(good >> k & 1u)) {
+      r[k] = first ? x1 : x2;
+      first = false;
+    }
+  S.done = good;
+  return S;
+}
+
+// One Newton step of root x on the quintic c.  kFloor: also compare the residual with the rounding floor of its own
+// evaluation.  Returns true when the root is converged (see the stop rule above); prev = |dx| of the previous step.
+template <bool kFloor>
+TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev) {
+  TWK_COUNT(newton_eval);
+  cd p = c[5], d = mk(0.0, 0.0);
+#pragma unroll
+  for (int i = 4; i >= 0; --i) {
+    d = cfma(d, x, p);
+    p = cfma(p, x, c[i]);
+  }
+  if (kFloor) {
+    const double ax = abs1(x);
+    double err = abs1(c[5]);
+#pragma unroll
+    for (int i = 4; i >= 0; --i) err = fma(err, ax, abs1(c[i]));
+    if (abs1(p) <= 2.0 * kEps * err) return true;   // at the rounding floor
+  }
+  const double dn = norm2(d);
+  if (!(dn > 0.0)) return false;
+  const cd dx = cdiv(p, d);
+  x = x - dx;
+  const double sdx = abs1(dx), ar = abs1(x);
+  const bool conv = sdx * sdx * sdx <= (0.125 * kEps) * ar * prev * prev || sdx <= kEps * ar;
+  prev = sdx;
+  return conv;
+}
+
 TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5]) {
   double prev[5];
 #pragma unroll
   for (int k = 0; k < 5; ++k) prev[k] = 0.0;
+  const cd tot = -cdiv(c[4], c[5]);   // sum of the five roots
   unsigned done = 0;
-  for (int it = 0; it < 12 && done != 31u; ++it) {
-    const bool floor_check = it >= 2;
+  // sweeps 0 and 1: every root needs them (the stop rule wants two steps), so all five chains run unconditionally
+  // and interleave (instruction-level parallelism); a step on an already converged root is harmless
+#pragma unroll
+  for (int it = 0; it < 2; ++it) {
+    unsigned dn = 0;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) dn |= newton_step<false>(c, r[k], prev[k]) ? (1u << k) : 0u;
+    done |= dn;
+  }
+  bool recovered = false;
+  for (int it = 2; it < 22; ++it) {
+    if (done == 31u || (it >= 10 && !recovered)) {
+      const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
+      if (done == 31u && abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale) return true;
+      if (recovered) break;
+      recovered = true;
+      SeededState S;
+#pragma unroll
+      for (int k = 0; k < 5; ++k) S.r[k] = r[k];
+      S.done = done;
+      S.ok = 0;
+      S = seeded_recover(c[0], c[5], tot, S);
+      if (!S.ok) break;
+#pragma unroll
+      for (int k = 0; k < 5; ++k)
+        if (!(S.done >> k & 1u)) {
+          r[k] = S.r[k];
+          prev[k] = 0.0;
+        }
+      done = S.done;
+    }
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
       if (done & (1u << k)) continue;
-      TWK_COUNT(newton_eval);
-      cd p = c[5], d = mk(0.0, 0.0);
-#pragma unroll
-      for (int i = 4; i >= 0; --i) {
-        d = cfma(d, r[k], p);
-        p = cfma(p, r[k], c[i]);
-      }
-      if (floor_check) {
-        const double ax = abs1(r[k]);
-        double err = abs1(c[5]);
-#pragma unroll
-        for (int i = 4; i >= 0; --i) err = fma(err, ax, abs1(c[i]));
-        if (abs1(p) <= 2.0 * kEps * err) { done |= 1u << k; continue; }   // at the rounding floor
-      }
-      const double dn = norm2(d);
-      if (!(dn > 0.0)) continue;
-      const cd dx = cdiv(p, d);
-      r[k] = r[k] - dx;
-      const double sdx = abs1(dx), ar = abs1(r[k]);
-      if (sdx * sdx * sdx <= (0.125 * kEps) * ar * prev[k] * prev[k] || sdx <= kEps * ar) done |= 1u << k;
-      prev[k] = sdx;
+      if (newton_step<true>(c, r[k], prev[k])) done |= 1u << k;
     }
   }
-  if (done != 31u) { TWK_COUNT(fail_iter); return false; }
-  // distinctness: sum of the roots against -c4/c5
-  const cd want = -cdiv(c[4], c[5]);
-  const cd sum = (r[0] + r[1]) + (r[2] + r[3]) + r[4];
-  const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
-  return abs1(sum - want) <= 1e-9 * scale;
+  TWK_COUNT(fail_iter);
+  return false;
 }
 
 }  // namespace twk
