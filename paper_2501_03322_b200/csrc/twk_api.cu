@@ -81,7 +81,30 @@ int cuda_fail(cudaError_t e) {
 
 }  // namespace
 
+// stage 1 with Q teams of 64 threads per CTA; resident CTAs per SM chosen so that 12 warps are resident
+template <int Q, int kMinBlocks>
+void launch_stage1_q(int sms, long long n_sources, const twk::Stage1Args& a, cudaStream_t stream) {
+  const long long groups = (n_sources + Q * twk::kS1Group - 1) / (Q * twk::kS1Group);
+  const size_t smem = twk::stage1_smem_bytes<Q>();
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(twk::stage1_kernel<Q, kMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_set = true;
+  }
+  const long long resident = (long long)sms * kMinBlocks;
+  const int grid = (int)(groups < resident ? groups : resident);
+  twk::stage1_kernel<Q, kMinBlocks><<<grid, Q * twk::kThreads, smem, stream>>>(a);
+}
+
+void launch_stage1(int teams, int sms, long long groups /* n_sources */, const twk::Stage1Args& a, cudaStream_t stream) {
+  // measured on config 3 (B200): 1 team x 6 CTAs/SM 36.5 ms, 2 x 3: 36.0, 3 x 2: 38.3, 4 x 1: 47.8, 6 x 1: 43.7 --
+  // coupling the teams through CTA-wide barriers costs more than the shared instruction stream saves
+  (void)teams;
+  launch_stage1_q<1, 6>(sms, groups, a, stream);
+}
+
 struct twk_ctx {
+  int stage1_teams;
   twk_options opt;
   size_t max_sources;
   int sms;
@@ -139,6 +162,7 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   c->last_launches = 0;
   c->timing = 0;
   c->ev_used = 0;
+  c->stage1_teams = 1;
   for (int i = 0; i < 5; ++i) c->ev[i] = nullptr;
   cudaError_t e = cudaMalloc((void**)&c->ws, c->lay.total);
   if (e != cudaSuccess) {
@@ -224,10 +248,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     a1.out_err = out_err;
     a1.out_nsamples = out_nsamples;
     a1.out_status = out_status;
-    const long long groups = ((long long)n_sources + twk::kThreads - 1) / twk::kThreads;
-    const long long resident = (long long)ctx->sms * 6;
-    const int grid = (int)(groups < resident ? groups : resident);
-    twk::stage1_kernel<<<grid, twk::kThreads, twk::stage1_smem_bytes(), stream>>>(a1);
+    launch_stage1(ctx->stage1_teams, ctx->sms, (long long)n_sources, a1, stream);
     ++launches;
     mark();
   }

@@ -142,7 +142,7 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     if (out_kind) out_kind[k] = (int8_t)kind[k];
     if (kind[k] != 0) {
       const int slot = (kind[k] > 0) ? sp++ : sm++;
-      const double invJ = 1.0 / J[k];
+      const double invJ = rcp(J[k]);
       // z' = (zeta' - conj(f') conj(zeta')) / J                       Eq.(10), repaired (E-2)
       const cd t = conj(fp[k]) * conj(dzeta);
       const cd zp = mk((dzeta.x - t.x) * invJ, (dzeta.y - t.y) * invJ);
@@ -244,7 +244,7 @@ TWK_HD void link_terms(const RecRef& A, const RecRef& B, int ka, int kb, double 
   const double dAp = 0.5 * (p1 + p2);
   dA += par * (trap + dAp);
   const double E1 = fabs(wA - wB) * dth3 * (1.0 / 48.0);                // Eq.(17)
-  const double E2 = 1.5 * fabs(dAp * (norm2(dz) / (dth2 * fabs(dotp(pA, pB))) - 1.0));
+  const double E2 = 1.5 * fabs(dAp * (norm2(dz) * rcp(dth2 * fabs(dotp(pA, pB))) - 1.0));
   const double E3 = 0.1 * fabs(dAp) * dth2;
   const double E4 = fabs(p1 - p2);
   err += (E1 + E2) + (E3 + E4);

@@ -50,12 +50,27 @@ TWK_HD double dotp(cd a, cd b) { return fma(a.x, b.x, a.y * b.y); }       // P:1
 TWK_HD cd cfma(cd a, cd b, cd c) {                                        // a*b + c
   return mk(fma(a.x, b.x, fma(-a.y, b.y, c.x)), fma(a.x, b.y, fma(a.y, b.x, c.y)));
 }
+// 1/x for a normal, finite x: the hardware's 20-bit estimate + two Newton steps (5 instructions, ~1 ulp) instead of
+// the IEEE-rounded division with its range checks (~12).  x = 0 or non-finite gives inf or NaN, which every caller
+// tolerates (guards on the denominator or the kPointNonFinite flag).
+TWK_HD double rcp(double x) {
+#ifdef __CUDA_ARCH__
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+#else
+  return 1.0 / x;
+#endif
+}
 TWK_HD cd crecip(cd a) {
-  const double inv = 1.0 / norm2(a);
+  const double inv = rcp(norm2(a));
   return mk(a.x * inv, -a.y * inv);
 }
 TWK_HD cd cdiv(cd a, cd b) {
-  const double inv = 1.0 / norm2(b);
+  const double inv = rcp(norm2(b));
   return mk(fma(a.x, b.x, a.y * b.y) * inv, fma(a.y, b.x, -(a.x * b.y)) * inv);
 }
 TWK_HD cd csqrt_(cd a) {   // principal square root
@@ -138,6 +153,9 @@ TWK_HD void coeffs_eq6(cd y, double s, double m2, cd c[6]) {
 // all five (removes deflation error).  All in registers; loops are compile-time bounded.
 // ------------------------------------------------------------------------------------------------------------
 constexpr double kEps = 2.220446049250313e-16;
+#ifndef TWK_STOP_FACTOR
+#define TWK_STOP_FACTOR 0.125   // Newton stop rule: predicted next step <= TWK_STOP_FACTOR * eps * |root|
+#endif
 
 template <int N>
 TWK_HD cd laguerre(const cd (&a)[N + 1], cd x) {
@@ -326,7 +344,7 @@ TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev) {
   const cd dx = cdiv(p, d);
   x = x - dx;
   const double sdx = abs1(dx), ar = abs1(x);
-  const bool conv = sdx * sdx * sdx <= (0.125 * kEps) * ar * prev * prev || sdx <= kEps * ar;
+  const bool conv = sdx * sdx * sdx <= (TWK_STOP_FACTOR * kEps) * ar * prev * prev || sdx <= kEps * ar;
   prev = sdx;
   return conv;
 }
@@ -339,7 +357,7 @@ TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5]) {
   unsigned done = 0;
   // sweeps 0 and 1: every root needs them (the stop rule wants two steps), so all five chains run unconditionally
   // and interleave (instruction-level parallelism); a step on an already converged root is harmless
-#pragma unroll
+#pragma unroll 1
   for (int it = 0; it < 2; ++it) {
     unsigned dn = 0;
 #pragma unroll
@@ -368,7 +386,7 @@ TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5]) {
         }
       done = S.done;
     }
-#pragma unroll
+#pragma unroll 1
     for (int k = 0; k < 5; ++k) {
       if (done & (1u << k)) continue;
       if (newton_step<true>(c, r[k], prev[k])) done |= 1u << k;

@@ -33,150 +33,185 @@ struct Stage1Args {
 };
 
 constexpr int kS1ParamRows = 8;   // s, m1, m2, z2, Re zc, Im zc, rho, status|valid
-__host__ __device__ inline size_t stage1_smem_bytes() {
-  return (size_t)(kRecDoubles * kThreads + kSeedDoubles * kThreads + kS1ParamRows * kThreads + 2 * kThreads + 8) * 8 +
-         (size_t)(2 * kThreads + 4) * 4 + kThreads;
+constexpr int kS1Group = 64;      // sources per team and group (one centre solve per thread)
+
+// Q teams of 64 threads per CTA.  A CTA takes a super-group of Q x 64 consecutive sources; team q owns sources
+// q*64 .. q*64+63 of it and keeps its own shared-memory state; only the barriers are CTA-wide, which keeps the teams
+// in step so that the warps of an SM run through the same ~35 KB of hot code together instead of streaming it at
+// a dozen different places (instruction fetch was the top stall of the one-team kernel).
+template <int Q>
+__host__ __device__ constexpr size_t stage1_smem_bytes() {
+  return (size_t)(Q * (kRecDoubles * kThreads + kSeedDoubles * kS1Group + kS1ParamRows * kS1Group + 2 * kS1Group) +
+                  2 * Q * 4) * 8 +
+         (size_t)(Q * 2 * kS1Group + 2 * Q * 2 + 2 * Q + 4) * 4 + Q * kS1Group;
 }
 
-// block-wide sum of two doubles and OR of an int over 64 threads (2 warps); result valid in every thread
-__device__ __forceinline__ void block_sum2_or(double& a, double& b, int& f, double* scratch /* >= 4 doubles */,
-                                              int* iscratch /* >= 2 ints */) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    a += __shfl_xor_sync(0xffffffffu, a, o);
-    b += __shfl_xor_sync(0xffffffffu, b, o);
-  }
-  f = __reduce_or_sync(0xffffffffu, (unsigned)f);
-  const int warp = threadIdx.x >> 5;
-  __syncthreads();
-  if ((threadIdx.x & 31) == 0) {
-    scratch[2 * warp] = a;
-    scratch[2 * warp + 1] = b;
-    iscratch[warp] = f;
-  }
-  __syncthreads();
-  a = scratch[0] + scratch[2];
-  b = scratch[1] + scratch[3];
-  f = iscratch[0] | iscratch[1];
-}
-
-__global__ void __launch_bounds__(kThreads, 6) stage1_kernel(Stage1Args p) {
+template <int Q, int kMinBlocks>
+__global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1Args p) {
   extern __shared__ double sm[];
-  double* recs = sm;                                   // [26][64]
-  double* seeds = recs + kRecDoubles * kThreads;       // [30][64]: seed block (twk_contour.cuh); column = source
-  double* prm = seeds + kSeedDoubles * kThreads;       // [8][64]
-  double* res_mu = prm + kS1ParamRows * kThreads;      // [64]
-  double* res_err = res_mu + kThreads;                 // [64]
-  double* scratch = res_err + kThreads;                // [8]
-  int* res_ns = reinterpret_cast<int*>(scratch + 8);   // [64]
-  int* res_st = res_ns + kThreads;                     // [64]
-  int* iscr = res_st + kThreads;                       // [4]
-  uint8_t* res_pend = reinterpret_cast<uint8_t*>(iscr + 4);   // [64]
-
-  const int t = threadIdx.x;
+  const int tid = threadIdx.x;
+  const int q = tid >> 6, t = tid & (kThreads - 1), warp = (tid >> 5) & 1;
+  double* recs_all = sm;                                                  // [Q][26][64]
+  double* seeds_all = recs_all + Q * kRecDoubles * kThreads;              // [Q][30][64] seed blocks; column = source
+  double* prm_all = seeds_all + Q * kSeedDoubles * kS1Group;              // [Q][8][64]
+  double* res_mu_all = prm_all + Q * kS1ParamRows * kS1Group;             // [Q][64]
+  double* res_err_all = res_mu_all + Q * kS1Group;                        // [Q][64]
+  double* scratch = res_err_all + Q * kS1Group;                           // [2 (round parity)][Q][2 warps][2]
+  int* res_ns_all = reinterpret_cast<int*>(scratch + 2 * Q * 4);          // [Q][64]
+  int* res_st_all = res_ns_all + Q * kS1Group;                            // [Q][64]
+  int* fscr = res_st_all + Q * kS1Group;                                  // [2][Q][2] flags of each warp
+  int* slots = fscr + 2 * Q * 2;                                          // [2][Q] hand-over slot of each team's source
+  int* iscr = slots + 2 * Q;                                              // [4]
+  uint8_t* res_pend_all = reinterpret_cast<uint8_t*>(iscr + 4);           // [Q][64]
+  double* recs = recs_all + q * kRecDoubles * kThreads;
+  double* seeds = seeds_all + q * kSeedDoubles * kS1Group;
+  double* prm = prm_all + q * kS1ParamRows * kS1Group;
+  double* res_mu = res_mu_all + q * kS1Group;
+  double* res_err = res_err_all + q * kS1Group;
+  int* res_ns = res_ns_all + q * kS1Group;
+  int* res_st = res_st_all + q * kS1Group;
+  uint8_t* res_pend = res_pend_all + q * kS1Group;
   double cs, sn;
   sincospi(double(t) / 32.0, &sn, &cs);   // theta_t = 2 pi t / 64 (reading A-3)
   const RecRef mine{recs + t, kThreads};
   const RecRef next{recs + ((t + 1) & (kThreads - 1)), kThreads};
   const long long n = p.b.n_sources;
-  const long long n_groups = (n + kThreads - 1) / kThreads;
+  const long long n_groups = (n + Q * kS1Group - 1) / (Q * kS1Group);   // super-groups
+  int parity = 0;
 
   for (;;) {
     __syncthreads();
-    if (t == 0) iscr[0] = atomicAdd(p.cursor, 1);
+    if (tid == 0) iscr[0] = atomicAdd(p.cursor, 1);
     __syncthreads();
     const long long g = iscr[0];
     if (g >= n_groups) break;
-    const long long base = g * kThreads;
+    const long long base = (g * Q + q) * kS1Group;   // first source of this team
     // ---- phase 1: parameters and centre roots of source base + t --------------------------------------------------
     {
       const long long src = base + t;
       if (src < n) {
         const SourceParams S = load_source(p.b, src);
-        prm[0 * kThreads + t] = S.L.s;
-        prm[1 * kThreads + t] = S.L.m1;
-        prm[2 * kThreads + t] = S.L.m2;
-        prm[3 * kThreads + t] = S.L.z2;
-        prm[4 * kThreads + t] = S.zc.x;
-        prm[5 * kThreads + t] = S.zc.y;
-        prm[6 * kThreads + t] = S.rho;
-        prm[7 * kThreads + t] = double((int)S.status | (S.valid ? 256 : 0));
-        if (S.valid) centre_seeds(S.L, S.zc, S.rho, seeds + t, kThreads);
+        prm[0 * kS1Group + t] = S.L.s;
+        prm[1 * kS1Group + t] = S.L.m1;
+        prm[2 * kS1Group + t] = S.L.m2;
+        prm[3 * kS1Group + t] = S.L.z2;
+        prm[4 * kS1Group + t] = S.zc.x;
+        prm[5 * kS1Group + t] = S.zc.y;
+        prm[6 * kS1Group + t] = S.rho;
+        prm[7 * kS1Group + t] = double((int)S.status | (S.valid ? 256 : 0));
+        if (S.valid) centre_seeds(S.L, S.zc, S.rho, seeds + t, kS1Group);
       }
     }
     __syncthreads();
-    // ---- phase 2: one source at a time, one thread per boundary sample ------------------------------------------------
-    const int cnt = (int)((n - base < kThreads) ? (n - base) : kThreads);
-    for (int i = 0; i < cnt; ++i) {
-      const int code = (int)prm[7 * kThreads + i];
-      if (!(code & 256)) {   // invalid parameters: NaN out, status 8 (uniform branch)
-        if (t == 0) {
+    // ---- phase 2: one source per team at a time, one thread per boundary sample ---------------------------------------
+    const int cnt = (int)((n - base < kS1Group) ? (n > base ? n - base : 0) : kS1Group);   // of this team
+    for (int i = 0; i < kS1Group; ++i) {
+      if (g * Q * kS1Group + i >= n) break;              // CTA-uniform: no team has a source i
+      const int code = (i < cnt) ? (int)prm[7 * kS1Group + i] : 0;
+      const bool active = (code & 256) != 0;            // team-uniform
+      double rho = 1.0;
+      int flags = 0;
+      if (active) {
+        Lens L;
+        L.s = prm[0 * kS1Group + i];
+        L.m1 = prm[1 * kS1Group + i];
+        L.m2 = prm[2 * kS1Group + i];
+        L.z2 = prm[3 * kS1Group + i];
+        const cd zc = mk(prm[4 * kS1Group + i], prm[5 * kS1Group + i]);
+        rho = prm[6 * kS1Group + i];
+        flags = point_solve_cs(L, zc, rho, cs, sn, seeds + i, kS1Group, mine, nullptr, nullptr, nullptr);
+      }
+      __syncthreads();                                   // records of every team complete
+      Piece P;
+      P.dA = 0.0;
+      P.err = 0.0;
+      if (active) P = eval_interval(mine, next, kTwoPi / double(kThreads));
+      // team sums: warp shuffle, then the two warps of the team through (double-buffered) shared memory
+      double A = P.dA, E = P.err;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        A += __shfl_xor_sync(0xffffffffu, A, o);
+        E += __shfl_xor_sync(0xffffffffu, E, o);
+      }
+      flags = (int)__reduce_or_sync(0xffffffffu, (unsigned)flags);
+      double* sc = scratch + parity * (Q * 4);
+      int* fs = fscr + parity * (Q * 2);
+      if ((tid & 31) == 0) {
+        sc[q * 4 + warp * 2] = A;
+        sc[q * 4 + warp * 2 + 1] = E;
+        fs[q * 2 + warp] = flags;
+      }
+      __syncthreads();
+      // every thread sees every team's sums: the decisions are CTA-uniform
+      bool any_pend = false, pend = false, finite = true;
+#pragma unroll
+      for (int qq = 0; qq < Q; ++qq) {
+        const double Aq = sc[qq * 4] + sc[qq * 4 + 2], Eq = sc[qq * 4 + 1] + sc[qq * 4 + 3];
+        const bool act = ((g * Q + qq) * kS1Group + i < n) && (((int)prm_all[(qq * kS1ParamRows + 7) * kS1Group + i]) & 256);
+        const bool fin = isfinite(Aq) && isfinite(Eq);
+        const bool pd = act && fin && !(Eq <= p.tol * fabs(Aq)) && !p.final_stage;   // stop rule P:272
+        any_pend = any_pend || pd;
+        if (qq == q) {
+          A = Aq;
+          E = Eq;
+          pend = pd;
+          finite = fin;
+        }
+      }
+      flags = fs[q * 2] | fs[q * 2 + 1];
+      if (any_pend) {
+        // a9: append to the refinement worklist; hand the first-iteration state over when a slot is free
+        int* sl = slots + parity * Q;
+        if (t == 0 && pend) {
+          const int slot = atomicAdd(p.list_count, 1);
+          p.list[slot] = (int32_t)(base + i);
+          sl[q] = slot;
+        }
+        __syncthreads();
+        if (pend) {
+          const long long slot = sl[q];
+          if (slot < p.handoff_slots) {
+            double* h = p.handoff + (size_t)slot * kHandDoubles;
+#pragma unroll
+            for (int e = 0; e < kRecDoubles; ++e) h[e * kThreads + t] = mine.at(e);
+            h[kRecDoubles * kThreads + t] = P.dA;
+            h[(kRecDoubles + 1) * kThreads + t] = P.err;
+            if (t < kSeedDoubles) h[(kRecDoubles + 2) * kThreads + t] = seeds[t * kS1Group + i];
+          }
+        }
+      }
+      if (t == 0 && i < cnt) {
+        if (!active) {   // invalid parameters: NaN out, status 8
           res_mu[i] = nan("");
           res_err[i] = nan("");
           res_ns[i] = 0;
           res_st[i] = 8;
           res_pend[i] = 0;
-        }
-        continue;
-      }
-      Lens L;
-      L.s = prm[0 * kThreads + i];
-      L.m1 = prm[1 * kThreads + i];
-      L.m2 = prm[2 * kThreads + i];
-      L.z2 = prm[3 * kThreads + i];
-      const cd zc = mk(prm[4 * kThreads + i], prm[5 * kThreads + i]);
-      const double rho = prm[6 * kThreads + i];
-      int flags = point_solve_cs(L, zc, rho, cs, sn, seeds + i, kThreads, mine, nullptr, nullptr, nullptr);
-      __syncthreads();
-      const Piece P = eval_interval(mine, next, kTwoPi / double(kThreads));
-      double A = P.dA, E = P.err;
-      block_sum2_or(A, E, flags, scratch, iscr + 1);
-      // every thread holds A, E: the decision is uniform
-      const bool finite = isfinite(A) && isfinite(E);
-      const bool pend = finite && !(E <= p.tol * fabs(A)) && !p.final_stage;   // stop rule P:272
-      if (pend) {
-        // a9: append to the refinement worklist; hand the first-iteration state over when a slot is free
-        if (t == 0) {
-          const int slot = atomicAdd(p.list_count, 1);
-          p.list[slot] = (int32_t)(base + i);
-          iscr[3] = slot;
-        }
-        __syncthreads();
-        const long long slot = iscr[3];
-        if (slot < p.handoff_slots) {
-          double* h = p.handoff + (size_t)slot * kHandDoubles;
-#pragma unroll
-          for (int e = 0; e < kRecDoubles; ++e) h[e * kThreads + t] = mine.at(e);
-          h[kRecDoubles * kThreads + t] = P.dA;
-          h[(kRecDoubles + 1) * kThreads + t] = P.err;
-          if (t < kSeedDoubles) h[(kRecDoubles + 2) * kThreads + t] = seeds[t * kThreads + i];
+        } else {
+          uint32_t status = (uint32_t)(code & 255);
+          if (!finite) status |= 16u;
+          else if (E <= p.tol * fabs(A)) status |= 1u;               // stop rule P:272
+          else if (p.final_stage) status |= 2u;                       // cap P:326
+          if (flags & kPointRepaired) status |= 4u;
+          if (flags & kPointNonFinite) status |= 16u;
+          res_mu[i] = A / (kPi * rho * rho);
+          res_err[i] = E / fabs(A);
+          res_ns[i] = kThreads;
+          res_st[i] = (int)status;
+          res_pend[i] = pend ? 1 : 0;
         }
       }
-      if (t == 0) {
-        uint32_t status = (uint32_t)(code & 255);
-        if (!finite) status |= 16u;
-        else if (E <= p.tol * fabs(A)) status |= 1u;               // stop rule P:272
-        else if (p.final_stage) status |= 2u;                       // cap P:326
-        if (flags & kPointRepaired) status |= 4u;
-        if (flags & kPointNonFinite) status |= 16u;
-        res_mu[i] = A / (kPi * rho * rho);
-        res_err[i] = E / fabs(A);
-        res_ns[i] = kThreads;
-        res_st[i] = (int)status;
-        res_pend[i] = pend ? 1 : 0;
-      }
+      parity ^= 1;
     }
     __syncthreads();
     // ---- phase 3: coalesced results -----------------------------------------------------------------------------------
     {
       const long long src = base + t;
-      if (src < n) {
-        if (!res_pend[t]) {
-          p.out_mu[src] = res_mu[t];
-          if (p.out_err) p.out_err[src] = res_err[t];
-          if (p.out_nsamples) p.out_nsamples[src] = res_ns[t];
-          if (p.out_status) p.out_status[src] = (uint32_t)res_st[t];
-        }
+      if (src < n && !res_pend[t]) {
+        p.out_mu[src] = res_mu[t];
+        if (p.out_err) p.out_err[src] = res_err[t];
+        if (p.out_nsamples) p.out_nsamples[src] = res_ns[t];
+        if (p.out_status) p.out_status[src] = (uint32_t)res_st[t];
       }
     }
   }

