@@ -27,9 +27,10 @@ sys.path.insert(0, ROOT)
 
 METRIC = "finite-source magnifications/sec at rel. acc 1e-4"
 UNIT = "magnifications/s"
-# FP64 flop per boundary point solve (a1-a7), executed-instruction count from the ncu capture in profiles/
-# (2*DFMA + DMUL + DADD per thread, stage-1 kernel, config 3) -- see DESIGN.md "Roofline".
-FLOP_PER_POINT = 4750.0
+# FP64 flop per boundary point (a1-a7: sample, coefficients, solve, lens quantities, ghost filter, its interval's
+# link + area + error), the executed-instruction count of the stage-1 kernel on config 3 from the ncu capture in
+# profiles/ (2*DFMA + DMUL + DADD thread instructions / boundary points) -- see DESIGN.md "Roofline".
+FLOP_PER_POINT = 2155.0
 FP64_LANES_PER_SM = 64          # FP64 FMA lanes per SM (derivation of the ALU peak)
 
 

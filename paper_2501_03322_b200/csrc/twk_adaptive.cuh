@@ -150,9 +150,10 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
             const int khi = min(kThreads, max(0, (int)ceil(cum_incl * scale - 0.5)));
             const double th0 = theta[i];
             const double hi = (i + 1 < n) ? theta[i + 1] : kTwoPi;
+            const double inv_w = rcp(w);
             for (int k = klo; k < khi; ++k) {
               const double target = (double(k) + 0.5) / double(kThreads) * W;
-              const double frac = (target - cum_excl) / w;
+              const double frac = (target - cum_excl) * inv_w;
               const double th = fma(frac, hi - th0, th0);              // linear interpolation
               newth[k] = (th > th0 && th < hi) ? th : nan("");
               newint[k] = i;
@@ -212,7 +213,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         ids[pos] = (uint16_t)(n + t);
         double sn, cs;
         if (n == 0) sincospi(double(t) / 32.0, &sn, &cs);   // exactly stage 1's angles
-        else sincos(th, &sn, &cs);
+        else sincospi(th * kInvPi, &sn, &cs);               // no range-reduction slow path
         flags |= point_solve_cs(S.L, S.zc, S.rho, cs, sn, seeds, 1, recref(n + t), nullptr, nullptr, nullptr);
       }
       const int n_new = n + m;

@@ -2,6 +2,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -99,8 +100,9 @@ void launch_stage1_q(int sms, long long n_sources, const twk::Stage1Args& a, cud
 void launch_stage1(int teams, int sms, long long groups /* n_sources */, const twk::Stage1Args& a, cudaStream_t stream) {
   // measured on config 3 (B200): 1 team x 6 CTAs/SM 36.5 ms, 2 x 3: 36.0, 3 x 2: 38.3, 4 x 1: 47.8, 6 x 1: 43.7 --
   // coupling the teams through CTA-wide barriers costs more than the shared instruction stream saves
-  (void)teams;
-  launch_stage1_q<1, 6>(sms, groups, a, stream);
+  if (teams == 24) launch_stage1_q<2, 4>(sms, groups, a, stream);
+  else if (teams == 2) launch_stage1_q<2, 3>(sms, groups, a, stream);
+  else launch_stage1_q<1, 6>(sms, groups, a, stream);
 }
 
 struct twk_ctx {
@@ -163,6 +165,7 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   c->timing = 0;
   c->ev_used = 0;
   c->stage1_teams = 1;
+  if (const char* e = getenv("TWK_STAGE1_TEAMS")) c->stage1_teams = atoi(e);
   for (int i = 0; i < 5; ++i) c->ev[i] = nullptr;
   cudaError_t e = cudaMalloc((void**)&c->ws, c->lay.total);
   if (e != cudaSuccess) {

@@ -19,6 +19,7 @@ namespace twk {
 
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr double kPi = 3.141592653589793238462643383279;
+constexpr double kInvPi = 0.318309886183790671537767526745;
 constexpr int kThreads = 64;   // threads per source = samples per iteration
 // Hand-over slot (stage 1 -> stage 2), in doubles: records [26][64] | dA [64] | err [64] | seed block [30] (+2 pad)
 constexpr int kHandDoubles = (kRecDoubles + 2) * kThreads + 32;
