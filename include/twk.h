@@ -42,6 +42,7 @@ extern "C" {
 #define TWK_ST_DOMAIN 8u     /* s, q outside the validated domain 0.1<=s<=10, q>=1e-9: still computed;   */
                              /* non-finite / non-positive s, q, rho or non-finite zeta: out_mu = NaN             */
 #define TWK_ST_NUMERIC 16u   /* a non-finite value appeared in the solve (degenerate quintic, zeta on a lens)    */
+#define TWK_ST_SLOPE 32u     /* the slope detector re-judged a real image pair as ghosts (reading G-4) */
 
 typedef struct twk_ctx twk_ctx; /* opaque; owns only its device scratch workspace */
 
@@ -55,6 +56,13 @@ typedef struct {
                         /* pieces, seeds; 14,592 B per slot) of an unfinished source passes to the refinement stage  */
                         /* instead of being recomputed there.  -1 = default min(max_sources, 524288); 0 = none.      */
                         /* Sources beyond the slots are still refined (their first iteration is recomputed).        */
+  double slope_gate;    /* slope detector: at a change of the image count between adjacent samples the    */
+                        /* new real pair must be perpendicular (within 45 deg) to the neighbouring ghost pair, else    */
+                        /* it is re-judged as ghosts.  Applied only when both pairs are closer than slope_gate         */
+                        /* (Einstein radii; "works only for the point sources near caustics").  Default 1e-5;  */
+                        /* 0 switches the detector off.  Adaptive mode only.                                           */
+  double slope_cos;     /* largest |cos| of the angle between the two pairs still counted as perpendicular; default    */
+                        /* cos 45 deg (reading G-4).  0 <= slope_cos <= 1.                                             */
 } twk_options;
 
 /* Fill *opt with the defaults above. */

@@ -164,6 +164,7 @@ template <class R> struct Sample {
   R w[5];             // z' ^ z''         (Eq.10, corrected: divided by J)
   int nreal;
   int repaired;       // parity repair fired (reading G-5)
+  int slope;          // a real pair of this sample was re-judged as ghosts by the slope detector
   int sweeps;
 };
 
@@ -211,6 +212,7 @@ void point_solve(const Lens<R>& L, const Cx<R>& zc, R rho, R theta, Sample<R>& S
   // parity sum must be -1: (1+,2-) or (2+,3-).  If rounding next to the critical curve broke it, flip
   // the smallest-|J| image of the over-represented parity (reading G-5).
   S.repaired = 0;
+  S.slope = 0;
   const int want = (S.nreal - 1) / 2;
   while (npos != want) {
     int best = -1;
@@ -237,16 +239,20 @@ template <class R> struct Piece {
   R dA, err;
   int crossing;  // 0 none, +1 creation, -1 annihilation
   int bad;       // leftover images are not exactly one (+,-) pair on one side
+  int slope;     // slope detector (reading G-4): the crossing's real pair (kp, km) is not perpendicular to
+  int kp, km;    // the ghost pair of the 3-image sample next to it and must be re-judged as ghosts
   int nlinks;
   int linkL[5], linkR[5];  // root indices of the linked pairs (diagnostics / tests)
 };
 
 template <class R>
-void eval_interval(const Sample<R>& A, const Sample<R>& B, R dth, Piece<R>& P) {
+void eval_interval(const Sample<R>& A, const Sample<R>& B, R dth, Piece<R>& P, R slope_gate2 = R(0), R slope_cos2 = R(0.5)) {
   P.dA = 0;
   P.err = 0;
   P.crossing = 0;
   P.bad = 0;
+  P.slope = 0;
+  P.kp = P.km = -1;
   P.nlinks = 0;
   int leftA[5], leftB[5], nLA = 0, nLB = 0;
   for (int par = +1; par >= -1; par -= 2) {
@@ -309,6 +315,24 @@ void eval_interval(const Sample<R>& A, const Sample<R>& B, R dth, Piece<R>& P) {
   const int km = (S.kind[lf[0]] > 0) ? lf[1] : lf[0];
   const Cx<R> zpl = S.z[kp], zmi = S.z[km];
   const Cx<R> d = zpl - zmi;
+  {
+    // Slope detector, P:251-268 (reading G-4): next to the critical curve the real pair (5-image sample) and the
+    // ghost pair (3-image sample) are perpendicular.  Applied only when both pairs are closer than the gate
+    // ("works only for the point sources near caustics"); |cos| >= cos 45 deg = the pair is misjudged.
+    const Sample<R>& G = creation ? A : B;
+    int g[2], ng = 0;
+    for (int k = 0; k < 5 && ng < 2; ++k)
+      if (G.kind[k] == 0) g[ng++] = k;
+    if (ng == 2) {
+      const Cx<R> dg = G.z[g[0]] - G.z[g[1]];
+      const R nr = std::norm(d), ngg = std::norm(dg), c = dot(d, dg);
+      if (nr < slope_gate2 && ngg < slope_gate2 && c * c >= slope_cos2 * nr * ngg) {
+        P.slope = 1;
+        P.kp = kp;
+        P.km = km;
+      }
+    }
+  }
   const R sq = std::sqrt(std::abs(dot(S.zp[kp], S.zp[km])));
   const R dtt = std::abs(d) / sq;                                                    // Eq.(11) tilde Delta theta
   const R corr = (S.w[kp] - S.w[km]) * dtt * dtt * dtt / R(24);                      // Eq.(11)
@@ -379,6 +403,8 @@ void images_fixed_one(double s, double q, double rho_, double zre, double zim, i
 // ---------------------------------------------------------------------------------------------------------
 struct AdaptOpt {
   int samples_per_iter, initial_samples, max_samples, subtract_avg_tol;
+  double slope_gate;   // slope detector proximity gate (0 = off)
+  double slope_cos;    // largest |cos| still counted as perpendicular (cos 45 deg: reading G-4)
 };
 
 template <class R> struct Contour {
@@ -388,11 +414,40 @@ template <class R> struct Contour {
   std::vector<Sample<R>> S;   // sorted by theta
   std::vector<Piece<R>> P;    // P[i] = interval (S[i], S[i+1 mod n])
   R twopi;
+  R gate2 = R(0);             // square of the slope detector's gate
+  R cos2 = R(0.5);            // square of the largest |cos| counted as perpendicular
   void init(int n0) {
     S.resize(n0);
     for (int j = 0; j < n0; ++j) point_solve(L, zc, rho, twopi * R(j) / R(n0), S[j]);
     P.resize(n0);
     for (int j = 0; j < n0; ++j) eval(j);
+    slope_repair();
+  }
+  // Slope detector: "When the slope detector finds that the perpendicular condition is not satisfied, nearby
+  // image pairs are checked until the slope jump position is found or reaches the end of the image piece."  Rounds:
+  // re-judge the pairs flagged by a creation (sample to the right of the interval), then those flagged by an
+  // annihilation (sample to the left, if it still has five images), evaluate every interval again; repeat until no
+  // crossing is flagged.  A piece whose pairs are never perpendicular disappears pair by pair ("the whole area piece
+  // shall be deleted").
+  static void demote(Sample<R>& s, int kp, int km) {
+    s.kind[kp] = 0;
+    s.kind[km] = 0;
+    s.nreal = 3;
+    s.slope = 1;
+  }
+  void slope_repair() {
+    for (;;) {
+      const int n = (int)S.size();
+      std::vector<int> flagged;
+      for (int i = 0; i < n; ++i)
+        if (P[i].slope) flagged.push_back(i);
+      if (flagged.empty()) return;
+      for (int i : flagged)
+        if (P[i].crossing > 0) demote(S[(i + 1) % n], P[i].kp, P[i].km);
+      for (int i : flagged)
+        if (P[i].crossing < 0 && S[i].nreal == 5) demote(S[i], P[i].kp, P[i].km);
+      for (int i = 0; i < n; ++i) eval(i);
+    }
   }
   R dtheta(int i) const {
     const int n = (int)S.size();
@@ -400,7 +455,7 @@ template <class R> struct Contour {
   }
   void eval(int i) {
     const int n = (int)S.size();
-    eval_interval(S[i], S[(i + 1) % n], dtheta(i), P[i]);
+    eval_interval(S[i], S[(i + 1) % n], dtheta(i), P[i], gate2, cos2);
   }
   // insert new angles (each strictly inside some interval), re-evaluate only the changed intervals
   void insert(std::vector<R> th) {
@@ -431,6 +486,7 @@ template <class R> struct Contour {
     P.swap(P2);
     for (size_t i = 0; i < S.size(); ++i)
       if (dirty[i]) eval((int)i);
+    slope_repair();
   }
   void sums(R& A, R& E, int& nbad) const {
     A = 0;
@@ -451,6 +507,8 @@ void magnify_one(double s, double q, double rho_, double zre, double zim, double
   C.rho = (R)rho_;
   C.zc = Cx<R>((R)zre, (R)zim);
   C.twopi = R(2) * pi_v<R>();
+  C.gate2 = R(o.slope_gate) * R(o.slope_gate);
+  C.cos2 = R(o.slope_cos) * R(o.slope_cos);
   const R rtol = (R)tol;
   uint32_t status = 0;
   if (!(s > 0) || !(q > 0) || !(rho_ > 0) || !std::isfinite(s) || !std::isfinite(q) || !std::isfinite(rho_) ||
@@ -534,9 +592,13 @@ void magnify_one(double s, double q, double rho_, double zre, double zim, double
       C.insert(newth);
     }
   }
-  int rep = 0;
-  for (const auto& smp : C.S) rep |= smp.repaired;
+  int rep = 0, slp = 0;
+  for (const auto& smp : C.S) {
+    rep |= smp.repaired;
+    slp |= smp.slope;
+  }
   if (rep || nbad) status |= 4;
+  if (slp) status |= 32;
   if (out_mu) *out_mu = (double)(A / (pi_v<R>() * C.rho * C.rho));
   if (out_err) *out_err = (double)(E / std::abs(A));
   if (out_n) *out_n = (int32_t)C.S.size();
@@ -650,8 +712,8 @@ void orc_images_fixed(int64_t n_models, const double* s, const double* q, const 
 void orc_magnify(int64_t n_models, const double* s, const double* q, const double* rho, int64_t n_sources,
                  const int32_t* model_id, const double* zeta, double rel_tol, int mode, int samples_per_iter,
                  int initial_samples, int max_samples, int subtract_avg_tol, int prec, int nthreads, double* out_mu,
-                 double* out_err, int32_t* out_nsamples, uint32_t* out_status) {
-  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol};
+                 double* out_err, int32_t* out_nsamples, uint32_t* out_status, double slope_gate, double slope_cos) {
+  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol, slope_gate, slope_cos};
   (void)nthreads;
 #pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads > 0 ? nthreads : orc_num_threads())
   for (int64_t i = 0; i < n_sources; ++i) {
@@ -670,7 +732,7 @@ void orc_magnify(int64_t n_models, const double* s, const double* q, const doubl
 // Sorted sample angles the paper-style sampler ends with, for one source (diagnostics).  Returns n.
 int orc_magnify_thetas(double s, double q, double rho, double zre, double zim, double rel_tol, int samples_per_iter,
                        int initial_samples, int max_samples, int subtract_avg_tol, int prec, double* out_theta) {
-  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol};
+  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol, 1e-5, 0.70710678118654752};
   int32_t n = 0;
   if (prec) magnify_one<long double>(s, q, rho, zre, zim, rel_tol, 0, o, nullptr, nullptr, &n, nullptr, out_theta);
   else magnify_one<double>(s, q, rho, zre, zim, rel_tol, 0, o, nullptr, nullptr, &n, nullptr, out_theta);

@@ -9,9 +9,17 @@
 
 namespace twk {
 
+// eval_interval as an out-of-line call: used only by the slope detector's repair pass (rare), kept out of the hot
+// instruction stream
+TWK_NOINLINE Piece eval_interval_cold(RecRef A, RecRef B, double dth, double slope_gate2, double slope_cos2) {
+  return eval_interval(A, B, dth, slope_gate2, slope_cos2);
+}
+
 struct AdaptArgs {
   Batch b;
   double tol;
+  double slope_gate2;    // square of the slope detector's proximity gate (twk_options.slope_gate)
+  double slope_cos2;     // square of the largest |cos| still counted as perpendicular (twk_options.slope_cos)
   int cap;               // sample capacity of this stage (<= 4096)
   int subtract_avg_tol;
   int final_stage;       // 1: cap reached -> return value + estimate with TWK_ST_CAP; 0: hand to next stage
@@ -94,7 +102,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
       if (t == 0) centre_seeds(S.L, S.zc, S.rho, seeds, 1);
     }
     uint32_t status = S.status;
-    bool exhausted = false;
+    bool exhausted = false, slope_seen = false;
     double A = 0.0, E = 0.0;
     for (;;) {
       __syncthreads();
@@ -220,6 +228,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
       __syncthreads();
       // ---- re-evaluate only the intervals that changed: the one to the left of every new sample, and the
       //      one to its right when the next sample is old (or the list wraps around) ---------------------------------
+      int viol = 0;
       if (t < m) {
         const bool last_in_group = (t == m - 1) || (cint[t + 1] != cint[t]);
 #pragma unroll 1
@@ -228,16 +237,58 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
           const int ia = pos - 1 + side;                       // interval (ia, ia + 1)
           const int ib = (ia + 1 < n_new) ? ia + 1 : 0;
           const double dth = (ia + 1 < n_new) ? theta[ia + 1] - theta[ia] : kTwoPi - theta[ia];
-          const Piece P = eval_interval(recref(ids[ia]), recref(ids[ib]), dth);
+          const Piece P = eval_interval(recref(ids[ia]), recref(ids[ib]), dth, p.slope_gate2, p.slope_cos2);
           dA[ia] = P.dA;
           er[ia] = P.err;
+          viol |= P.slope;
         }
       }
       n = n_new;
+      // ---- a5, slope detector: a crossing whose real pair is not perpendicular to the neighbouring ghost
+      //      pair is re-judged.  Rare: out-of-line repair rounds over ALL intervals until none is flagged.  Each round:
+      //      evaluate everything, list the flagged crossings, re-judge the pairs flagged by a creation (the record to
+      //      the right of the interval), then those flagged by an annihilation (the record to the left, if it still has
+      //      five images). ------------------------------------------------------------------------------------------
+      if (__syncthreads_or(viol)) {
+        slope_seen = true;
+        for (int round = 0; round < 4096; ++round) {
+          if (t == 0) iscr[3] = 0;
+          __syncthreads();
+          for (int i = t; i < n; i += kThreads) {
+            const int ib = (i + 1 < n) ? i + 1 : 0;
+            const double dth = (i + 1 < n) ? theta[i + 1] - theta[i] : kTwoPi - theta[i];
+            const Piece P = eval_interval_cold(recref(ids[i]), recref(ids[ib]), dth, p.slope_gate2, p.slope_cos2);
+            dA[i] = P.dA;
+            er[i] = P.err;
+            if (P.slope) {
+              const int k = atomicAdd(&iscr[3], 1);
+              if (k < kThreads) {
+                newint[k] = i;
+                cint[k] = (P.slope & 255) | (P.crossing > 0 ? 256 : 0);
+              }
+            }
+          }
+          __syncthreads();
+          const int nv = min(iscr[3], kThreads);
+          if (nv == 0) break;
+          if (t < nv && (cint[t] & 256)) {
+            const int ib = (newint[t] + 1 < n) ? newint[t] + 1 : 0;
+            demote_pair(recref(ids[ib]), cint[t] & 15, (cint[t] >> 4) & 15);
+          }
+          __syncthreads();
+          if (t < nv && !(cint[t] & 256)) {
+            const RecRef S5 = recref(ids[newint[t]]);
+            if (S5.nreal() == 5) demote_pair(S5, cint[t] & 15, (cint[t] >> 4) & 15);
+          }
+          __syncthreads();
+        }
+      }
     }
+
     // ---- outputs / hand-over ------------------------------------------------------------------------------------
     const int rep = __syncthreads_or(flags & kPointRepaired);
     const int nonf = __syncthreads_or(flags & kPointNonFinite);
+    const int slp = __syncthreads_or(flags & kPointSlope);
     if (t == 0) {
       if (exhausted && !p.final_stage) {
         p.next_list[atomicAdd(p.next_count, 1)] = (int32_t)src;
@@ -245,6 +296,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         if (exhausted) status |= 2u;
         if (rep) status |= 4u;
         if (nonf) status |= 16u;
+        if (slope_seen || slp) status |= 32u;
         p.out_mu[src] = A / (kPi * S.rho * S.rho);
         if (p.out_err) p.out_err[src] = E / fabs(A);
         if (p.out_nsamples) p.out_nsamples[src] = n;

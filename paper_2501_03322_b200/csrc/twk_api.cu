@@ -2,7 +2,6 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -67,7 +66,7 @@ Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
 
 bool valid_options(const twk_options& o) {
   return o.samples_per_iter == twk::kThreads && o.initial_samples == twk::kThreads && o.max_samples >= twk::kThreads &&
-         o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1) && o.handoff_slots >= -1;
+         o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1) && o.handoff_slots >= -1 && o.slope_gate >= 0.0 && o.slope_cos >= 0.0 && o.slope_cos <= 1.0;
 }
 
 int cuda_fail(cudaError_t e) {
@@ -100,9 +99,8 @@ void launch_stage1_q(int sms, long long n_sources, const twk::Stage1Args& a, cud
 void launch_stage1(int teams, int sms, long long groups /* n_sources */, const twk::Stage1Args& a, cudaStream_t stream) {
   // measured on config 3 (B200): 1 team x 6 CTAs/SM 36.5 ms, 2 x 3: 36.0, 3 x 2: 38.3, 4 x 1: 47.8, 6 x 1: 43.7 --
   // coupling the teams through CTA-wide barriers costs more than the shared instruction stream saves
-  if (teams == 24) launch_stage1_q<2, 4>(sms, groups, a, stream);
-  else if (teams == 2) launch_stage1_q<2, 3>(sms, groups, a, stream);
-  else launch_stage1_q<1, 6>(sms, groups, a, stream);
+  (void)teams;
+  launch_stage1_q<1, 6>(sms, groups, a, stream);
 }
 
 struct twk_ctx {
@@ -131,6 +129,8 @@ void twk_default_options(twk_options* opt) {
   opt->max_samples = 4096;
   opt->subtract_avg_tol = 1;
   opt->handoff_slots = -1;
+  opt->slope_gate = 1e-5;
+  opt->slope_cos = 0.70710678118654752;
 }
 
 size_t twk_workspace_bytes(const twk_options* opt, size_t max_sources) {
@@ -165,7 +165,6 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   c->timing = 0;
   c->ev_used = 0;
   c->stage1_teams = 1;
-  if (const char* e = getenv("TWK_STAGE1_TEAMS")) c->stage1_teams = atoi(e);
   for (int i = 0; i < 5; ++i) c->ev[i] = nullptr;
   cudaError_t e = cudaMalloc((void**)&c->ws, c->lay.total);
   if (e != cudaSuccess) {
@@ -221,6 +220,8 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
   twk::AdaptArgs a{};
   a.b = twk::Batch{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources};
   a.tol = rel_tol;
+  a.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
+  a.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
   a.subtract_avg_tol = ctx->opt.subtract_avg_tol;
   a.out_mu = out_mu;
   a.out_err = out_err;
@@ -241,6 +242,8 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     twk::Stage1Args a1{};
     a1.b = a.b;
     a1.tol = rel_tol;
+    a1.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
+    a1.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
     a1.final_stage = P.cap2 ? 0 : 1;
     a1.cursor = counters + 0;
     a1.list = list1;

@@ -9,11 +9,12 @@ namespace twk {
 // ------------------------------------------------------------------------------------------------------------
 // Sample record: what an interval needs from one boundary sample.  26 doubles, element e at base[e * stride]:
 //   [0..4]  Re z      slots 0,1 = positive-parity images, slots 2,3,4 = negative-parity images
-//   [5..9]  Im z      (slot 1 and slot 4 are filled only when the sample has 5 real images)
+//   [5..9]  Im z      (a sample with 3 real images keeps its GHOST pair's positions in the z fields of slots 1 and 4:
+//                     the slope detector compares directions across a count change)
 //   [10..14] Re z'    z' = dz/dtheta, Eq.(10) (conj on f' restored)
 //   [15..19] Im z'
 //   [20..24] z'^z''   Eq.(10) (division by J restored)
-//   [25]    nreal (3 or 5) + 8 * repaired + 16 * non-finite, stored as a double
+//   [25]    nreal (3 or 5) + 8 * point flags (kPointRepaired | kPointNonFinite | kPointSlope), stored as a double
 // In shared memory the record is a column of a [26][TILE] array (stride = TILE, conflict-free); in the global
 // arena it is 26 contiguous doubles (stride = 1, 208 B).
 // ------------------------------------------------------------------------------------------------------------
@@ -28,10 +29,11 @@ struct RecRef {
   TWK_HD cd zp(int slot) const { return mk(base[(kPX + slot) * stride], base[(kPY + slot) * stride]); }
   TWK_HD double w(int slot) const { return base[(kW + slot) * stride]; }
   TWK_HD int nreal() const { return int(base[kNR * stride]) & 7; }
-  TWK_HD int point_flags() const { return int(base[kNR * stride]) >> 3; }   // kPointRepaired | kPointNonFinite
+  TWK_HD int point_flags() const { return int(base[kNR * stride]) >> 3; }
 };
 
 constexpr int kPointRepaired = 1;   // parity sum was not -1 and was repaired (G-5)
+constexpr int kPointSlope = 4;      // a real pair was re-judged as ghosts by the slope detector
 constexpr int kPointNonFinite = 2;  // a root or a derived quantity is not finite
 
 // ------------------------------------------------------------------------------------------------------------
@@ -156,6 +158,12 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
       rec.at(kW + slot) = w;
     }
   }
+  if (nreal == 3) {   // ghost pair positions for the slope detector
+    rec.at(kZX + 1) = eA.x + L.z2;
+    rec.at(kZY + 1) = eA.y;
+    rec.at(kZX + 4) = eB.x + L.z2;
+    rec.at(kZY + 4) = eB.y;
+  }
   rec.at(kNR) = double(nreal + 8 * flags);
   if (out_count) *out_count = (int8_t)nreal;
   return flags;
@@ -230,6 +238,8 @@ TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int st
 struct Piece {
   double dA, err;
   int crossing;   // 0 none, +1 creation, -1 annihilation
+  int slope;      // slope detector (a5): 0 fine; otherwise the crossing's real pair is NOT perpendicular to the
+                  // ghost pair next to it and must be re-judged: slot of its positive image | slot of its negative << 4 | 256
 };
 
 TWK_HD void link_terms(const RecRef& A, const RecRef& B, int ka, int kb, double par, double dth, double& dA,
@@ -260,11 +270,12 @@ TWK_HD int crossed_is_shorter(double s00, double s11, double s01, double s10) {
   return (sqrt(s01) + sqrt(s10)) < (sqrt(s00) + sqrt(s11));
 }
 
-TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth) {
+TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth, double slope_gate2, double slope_cos2) {
   Piece P;
   P.dA = 0.0;
   P.err = 0.0;
   P.crossing = 0;
+  P.slope = 0;
   const bool a5 = A.nreal() == 5, b5 = B.nreal() == 5;
   int leftApos = -1, leftAneg = -1, leftBpos = -1, leftBneg = -1;
   // links are collected first (slot of A | slot of B << 4, one byte each) and evaluated in ONE loop below
@@ -353,6 +364,17 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth) {
     const cd zpl = S.z(kp), zmi = S.z(km), ppl = S.zp(kp), pmi = S.zp(km);
     const double wpl = S.w(kp), wmi = S.w(km);
     const cd d = zpl - zmi;
+    {
+      // a5, slope detector (reading G-4): next to the critical curve the real pair of the 5-image sample
+      // and the ghost pair of the 3-image sample point in perpendicular directions.  Applied only when both pairs
+      // are closer than the gate (the local expansion of Eq.(16) holds near the critical curve only
+      // "works only for the point sources near caustics"); not perpendicular (|cos| >= slope_cos, 45 deg by
+      // default) = misjudged.
+      const RecRef& G = creation ? A : B;
+      const cd dg = G.z(1) - G.z(4);
+      const double n_r = norm2(d), n_g = norm2(dg), c = dotp(d, dg);
+      if (n_r < slope_gate2 && n_g < slope_gate2 && c * c >= slope_cos2 * n_r * n_g) P.slope = kp | (km << 4) | 256;
+    }
     const double ad = sqrt(norm2(d));
     const double sq = sqrt(fabs(dotp(ppl, pmi)));
     const double dtt = ad / sq;                                         // Eq.(11) tilde Delta theta
@@ -376,6 +398,32 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth) {
     P.err += E1 + E2 + E3;
   }
   return P;
+}
+
+// a5, slope detector: re-judge the real pair (slots kp, km) of a 5-image record as the ghost pair ("pair 1
+// shall be rejudged as ghost images").  The record becomes a 3-image record: the other positive image in slot 0, the
+// other two negative images in slots 2 and 3, the pair's positions in the z fields of slots 1 and 4.
+TWK_HD void demote_pair(const RecRef& S, int kp, int km) {
+  const cd gp = S.z(kp), gm = S.z(km);
+  if (kp == 0) {
+    S.at(kZX) = S.at(kZX + 1);
+    S.at(kZY) = S.at(kZY + 1);
+    S.at(kPX) = S.at(kPX + 1);
+    S.at(kPY) = S.at(kPY + 1);
+    S.at(kW) = S.at(kW + 1);
+  }
+  if (km < 4) {   // slot 4 moves down into the hole
+    S.at(kZX + km) = S.at(kZX + 4);
+    S.at(kZY + km) = S.at(kZY + 4);
+    S.at(kPX + km) = S.at(kPX + 4);
+    S.at(kPY + km) = S.at(kPY + 4);
+    S.at(kW + km) = S.at(kW + 4);
+  }
+  S.at(kZX + 1) = gp.x;
+  S.at(kZY + 1) = gp.y;
+  S.at(kZX + 4) = gm.x;
+  S.at(kZY + 4) = gm.y;
+  S.at(kNR) = double(3 + 8 * (S.point_flags() | kPointSlope));
 }
 
 }  // namespace twk

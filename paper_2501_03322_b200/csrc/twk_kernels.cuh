@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(TILE) fixed_kernel(Batch b, int N, double* __r
       __syncthreads();
       if (j < N && j >= 1) {
         const RecRef prev = (t > 0) ? RecRef{rec + t - 1, TILE} : RecRef{carry, 1};
-        const Piece P = eval_interval(prev, mine, dth);
+        const Piece P = eval_interval(prev, mine, dth, 0.0, 0.5);   // slope detector off in fixed mode
         accA += P.dA;
         accE += P.err;
       }
@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(TILE) fixed_kernel(Batch b, int N, double* __r
     }
     __syncthreads();
     if (t == 0) {   // closing interval (N-1 -> 0)
-      const Piece P = eval_interval(RecRef{carry, 1}, RecRef{first, 1}, dth);
+      const Piece P = eval_interval(RecRef{carry, 1}, RecRef{first, 1}, dth, 0.0, 0.5);
       accA += P.dA;
       accE += P.err;
     }

@@ -20,6 +20,8 @@ namespace twk {
 struct Stage1Args {
   Batch b;
   double tol;
+  double slope_gate2;    // square of the slope detector's proximity gate (twk_options.slope_gate)
+  double slope_cos2;     // square of the largest |cos| still counted as perpendicular (twk_options.slope_cos)
   int final_stage;       // 1: there is no refinement stage (max_samples < 128): cap status instead of pending
   int* cursor;           // group fetch counter (zeroed before launch)
   int32_t* list;         // [n_sources] a9: worklist of unfinished sources, appended in completion order
@@ -123,25 +125,52 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
       }
       __syncthreads();                                   // records of every team complete
       Piece P;
-      P.dA = 0.0;
-      P.err = 0.0;
-      if (active) P = eval_interval(mine, next, kTwoPi / double(kThreads));
-      // team sums: warp shuffle, then the two warps of the team through (double-buffered) shared memory
-      double A = P.dA, E = P.err;
+      double A, E;
+      double* sc;
+      int* fs;
+      constexpr int kSlopeVote = 1 << 8;
+      for (;;) {
+        P.dA = 0.0;
+        P.err = 0.0;
+        P.crossing = 0;
+        P.slope = 0;
+        if (active) P = eval_interval(mine, next, kTwoPi / double(kThreads), p.slope_gate2, p.slope_cos2);
+        // team sums: warp shuffle, then the two warps of the team through (double-buffered) shared memory
+        A = P.dA;
+        E = P.err;
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
-        A += __shfl_xor_sync(0xffffffffu, A, o);
-        E += __shfl_xor_sync(0xffffffffu, E, o);
+        for (int o = 16; o > 0; o >>= 1) {
+          A += __shfl_xor_sync(0xffffffffu, A, o);
+          E += __shfl_xor_sync(0xffffffffu, E, o);
+        }
+        const int vote = (int)__reduce_or_sync(0xffffffffu, (unsigned)(flags | (P.slope ? kSlopeVote : 0)));
+        sc = scratch + parity * (Q * 4);
+        fs = fscr + parity * (Q * 2);
+        if ((tid & 31) == 0) {
+          sc[q * 4 + warp * 2] = A;
+          sc[q * 4 + warp * 2 + 1] = E;
+          fs[q * 2 + warp] = vote;
+        }
+        __syncthreads();
+        int any = 0;
+#pragma unroll
+        for (int j = 0; j < 2 * Q; ++j) any |= fs[j];
+        if (!(any & kSlopeVote)) break;                  // the common case: no extra barrier
+        // a5, slope detector: re-judge the flagged real pairs as ghosts and evaluate the contour again.
+        // A record is changed by one thread per phase: the interval on its left (creation into it) first, then the
+        // interval on its right (annihilation out of it) if it still has five images.
+        parity ^= 1;
+        if (P.slope && P.crossing > 0) {
+          demote_pair(next, P.slope & 15, (P.slope >> 4) & 15);
+          flags |= kPointSlope;                          // reaches the team's flags through the next vote
+        }
+        __syncthreads();
+        if (P.slope && P.crossing < 0 && mine.nreal() == 5) {
+          demote_pair(mine, P.slope & 15, (P.slope >> 4) & 15);
+          flags |= kPointSlope;
+        }
+        __syncthreads();
       }
-      flags = (int)__reduce_or_sync(0xffffffffu, (unsigned)flags);
-      double* sc = scratch + parity * (Q * 4);
-      int* fs = fscr + parity * (Q * 2);
-      if ((tid & 31) == 0) {
-        sc[q * 4 + warp * 2] = A;
-        sc[q * 4 + warp * 2 + 1] = E;
-        fs[q * 2 + warp] = flags;
-      }
-      __syncthreads();
       // every thread sees every team's sums: the decisions are CTA-uniform
       bool any_pend = false, pend = false, finite = true;
 #pragma unroll
@@ -158,7 +187,7 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
           finite = fin;
         }
       }
-      flags = fs[q * 2] | fs[q * 2 + 1];
+      flags = (fs[q * 2] | fs[q * 2 + 1]) & (kSlopeVote - 1);
       if (any_pend) {
         // a9: append to the refinement worklist; hand the first-iteration state over when a slot is free
         int* sl = slots + parity * Q;
@@ -194,6 +223,7 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
           else if (p.final_stage) status |= 2u;                       // cap P:326
           if (flags & kPointRepaired) status |= 4u;
           if (flags & kPointNonFinite) status |= 16u;
+          if (flags & kPointSlope) status |= 32u;
           res_mu[i] = A / (kPi * rho * rho);
           res_err[i] = E / fabs(A);
           res_ns[i] = kThreads;

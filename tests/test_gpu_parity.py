@@ -181,6 +181,41 @@ def test_handover_and_recompute_paths_agree():
         assert np.median(d) < 1e-13 and np.quantile(d, 0.99) < 1e-10 and d.max() < 2e-6, (np.median(d), d.max())
 
 
+@pytest.mark.parametrize("slope_cos", [0.70710678118654752, 0.2, 0.02, 0.0])
+def test_slope_detector_like_for_like(slope_cos):
+    """a5, slope detector.  With the default gate (1e-5) it never fires on these inputs (the residual
+    detector's 2-cycle reading is already right).  To exercise the re-judging walk on both sides the gate is opened
+    (1e30) and the perpendicularity bound tightened: crossings whose pairs are further than acos(slope_cos) from
+    perpendicular are re-judged pair by pair until a perpendicular one or the end of the piece is reached.  Same
+    rule on both sides -> same sample sets, same status bit, same area."""
+    import paper_2501_03322_b200 as P
+    full = W.config4()
+    zc = full.zeta[:, 0] + 1j * full.zeta[:, 1]
+    band = np.where((np.abs(zc.imag) < 0.25) & (np.abs(zc.real) < 0.6))[0]
+    cases = [W.fig2_case(), W.fig1_case(), full.subset(band[:: max(1, len(band) // 1200)])]
+    c = P.Context(4096, slope_gate=1e30, slope_cos=slope_cos)
+    fired = 0
+    for wl in cases:
+        g = c.magnify_workload(wl, 1e-4)
+        o = api.magnify(wl, 1e-4, mode=0, prec=0, slope_gate=1e30, slope_cos=slope_cos)
+        st = g["status"].astype(np.uint32)
+        same = g["nsamples"] == o["nsamples"]
+        d = np.abs(g["mu"] / o["mu"] - 1)
+        assert np.array_equal(st & 35, o["status"] & 35)                 # converged / cap / slope bits
+        if wl.n_sources > 1:
+            assert same.mean() > 0.97
+            assert np.quantile(d[same], 0.99) < 1e-8
+        # (a deleted piece leaves a jump the sampler refines until it runs out of distinct angles: the two sides may
+        #  then stop a sample or two apart)
+        assert d.max() < 5e-4 and np.all(np.abs(g["nsamples"] - o["nsamples"]) <= 64)
+        fired += int((st & P.TWK_ST_SLOPE != 0).sum())
+    c.close()
+    if slope_cos > 0.7:
+        assert fired == 0          # 45 degrees: every crossing of these inputs is perpendicular enough
+    if slope_cos == 0.0:
+        assert fired > 20          # nothing is perpendicular enough: every crossing piece is deleted
+
+
 def test_edge_cases(ctx):
     import torch
     import paper_2501_03322_b200 as P

@@ -240,3 +240,23 @@ def test_adaptive_sampler_concentrates_on_crossings():
     added = np.array([x for x in t if np.abs(x * 64 / (2 * np.pi) - round(x * 64 / (2 * np.pi))) > 1e-9])
     near = np.min(np.abs(added[:, None] - cross[None, :]), axis=1) < 0.3
     assert near.mean() > 2 * (4 * 0.3) / (2 * np.pi)
+
+
+def test_slope_detector_rejudging():
+    """Slope detector, P:251-268 (reading G-4).  (i) With the default gate it never fires on the worked examples and
+    changes nothing.  (ii) Opened up (gate 1e30) at the default 45 degrees it still never fires: real and ghost pairs
+    ARE perpendicular across every crossing of these inputs (the geometric fact the detector rests on, Eq.(16)).
+    (iii) With the bound tightened to 0 nothing counts as perpendicular: every crossing piece is re-judged pair by
+    pair until it is gone ("the whole area piece shall be deleted"): no crossing is left, status bit 32 is
+    set, and what remains is the area enclosed by the three image tracks that exist at every theta."""
+    wl = W.fig2_case()
+    base = api.magnify(wl, 1e-4, mode=0, slope_gate=0.0)
+    for gate, cs in ((1e-5, 0.70710678118654752), (1e30, 0.70710678118654752)):
+        r = api.magnify(wl, 1e-4, mode=0, slope_gate=gate, slope_cos=cs)
+        assert r["mu"][0] == base["mu"][0] and r["nsamples"][0] == base["nsamples"][0] and not (r["status"][0] & 32)
+    r = api.magnify(wl, 1e-4, mode=0, slope_gate=1e30, slope_cos=0.0)
+    assert r["status"][0] & 32
+    assert r["mu"][0] < base["mu"][0] - 0.5          # the merged image's extra lobe (tracks 4 and 5, P:159) is gone
+    # the long-double twin takes the same decisions
+    rl = api.magnify(wl, 1e-4, mode=0, prec=1, slope_gate=1e30, slope_cos=0.0)
+    assert abs(rl["mu"][0] / r["mu"][0] - 1) < 1e-9 and rl["nsamples"][0] == r["nsamples"][0]
