@@ -31,6 +31,9 @@ UNIT = "magnifications/s"
 # link + area + error), the executed-instruction count of the stage-1 kernel on config 3 from the ncu capture in
 # profiles/ (2*DFMA + DMUL + DADD thread instructions / boundary points) -- see DESIGN.md "Roofline".
 FLOP_PER_POINT = 2155.0
+# DRAM bytes of one stage-1 launch on config 3 (dram__bytes_read.sum + dram__bytes_write.sum of the same capture,
+# profiles/r01b_ncu_full.csv): 0.10 GB read + 4.05 GB written, of which 4.0 GB is the hand-over arena
+STAGE1_DRAM_BYTES_CONFIG3 = 4.147e9
 FP64_LANES_PER_SM = 64          # FP64 FMA lanes per SM (derivation of the ALU peak)
 
 
@@ -259,7 +262,10 @@ def main():
             "gpu_launches": stats["n_launches"] * args.steps,
             "clocks": clocks,
             "roofline": {"bound": "alu", "kernel": "stage1_kernel (64 point solves + 64 intervals per source)",
-                         "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf, "traffic": None,
+                         "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
+                         "traffic": STAGE1_DRAM_BYTES_CONFIG3 if wl.name == "config3" else None,
+                         "traffic_note": "DRAM bytes per stage-1 launch from profiles/r01b_ncu_full.csv; algorithmic "
+                                         "bytes are 45 B/source = 0.18 GB, the rest is the hand-over arena to stage 2",
                          "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x "
                                         f"{sm_max_mhz:.0f} MHz (MEASURED_PEAKS.json has no FP64 figure)",
                          "peak_probe_tflops": probe_tf, "frac_of_probe": achieved / probe_tf,
