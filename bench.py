@@ -49,10 +49,12 @@ def parse_args():
     return ap.parse_args()
 
 
-def make_workload(name, rank):
+def make_workload(name, rank, **size):
+    """The batch of rank `rank`: every rank draws its own seeded batch (independent problems, no collective on the
+    data path -- P:392 "no communication between devices")."""
     import workloads as W
     if name == "config3":
-        return W.config3(seed=250103322 + rank)
+        return W.config3(seed=250103322 + rank, **size)
     if name == "config5":
         return W.config5(seed=250103323 + rank)
     return W.get(name)
@@ -118,6 +120,16 @@ def cpu_baseline(wl, n_sample, tol):
             "sample": f"{n_sample} seeded-random sources of {wl.name} (of {wl.n_sources}), oracle paper-style sampler, "
                       f"double, tol {tol:g}, {dt:.1f} s wall, mean {float(r['nsamples'].mean()):.1f} samples/source",
             "seconds": dt}
+
+
+def max_over_ranks(values, device, world):
+    """Timing reduction of the N > 1 run: element-wise MAX over ranks (the only collective of the bench)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
 
 
 def run_reference(args):
@@ -228,10 +240,7 @@ def main():
     ms_e2e = f0.elapsed_time(f1)
     assert torch.equal(ho["mu"], out["out_mu"].cpu()), "host-buffer path and device path disagree"
 
-    t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e = float(t[0]), float(t[1])
+    ms, ms_e2e = max_over_ranks([ms, ms_e2e], dev, world)
 
     if rank == 0:
         peaks = {}
