@@ -83,15 +83,19 @@ int cuda_fail(cudaError_t e) {
 
 // stage 1 with Q teams of 64 threads per CTA; resident CTAs per SM chosen so that 12 warps are resident
 template <int Q, int kMinBlocks>
-void launch_stage1_q(int sms, long long n_sources, const twk::Stage1Args& a, cudaStream_t stream) {
-  const long long groups = (n_sources + Q * twk::kS1Group - 1) / (Q * twk::kS1Group);
+void launch_stage1_q(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t stream) {
   const size_t smem = twk::stage1_smem_bytes<Q>();
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(twk::stage1_kernel<Q, kMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_set = true;
   }
+  // groups of up to 64 sources per CTA pass; a small batch takes smaller groups so that every resident CTA gets work
   const long long resident = (long long)sms * kMinBlocks;
+  long long group = (n_sources + resident * Q - 1) / (resident * Q);
+  group = group < 4 ? 4 : (group > twk::kS1Group ? twk::kS1Group : group);
+  a.group = (int)group;
+  const long long groups = (n_sources + Q * group - 1) / (Q * group);
   const int grid = (int)(groups < resident ? groups : resident);
   twk::stage1_kernel<Q, kMinBlocks><<<grid, Q * twk::kThreads, smem, stream>>>(a);
 }

@@ -22,6 +22,7 @@ struct Stage1Args {
   double tol;
   double slope_gate2;    // square of the slope detector's proximity gate (twk_options.slope_gate)
   double slope_cos2;     // square of the largest |cos| still counted as perpendicular (twk_options.slope_cos)
+  int group;             // sources per group, 1..64 (smaller for small batches: more CTAs get work)
   int final_stage;       // 1: there is no refinement stage (max_samples < 128): cap status instead of pending
   int* cursor;           // group fetch counter (zeroed before launch)
   int32_t* list;         // [n_sources] a9: worklist of unfinished sources, appended in completion order
@@ -78,7 +79,8 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
   const RecRef mine{recs + t, kThreads};
   const RecRef next{recs + ((t + 1) & (kThreads - 1)), kThreads};
   const long long n = p.b.n_sources;
-  const long long n_groups = (n + Q * kS1Group - 1) / (Q * kS1Group);   // super-groups
+  const int G = p.group;
+  const long long n_groups = (n + Q * G - 1) / (Q * G);   // super-groups
   int parity = 0;
 
   for (;;) {
@@ -87,11 +89,11 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
     __syncthreads();
     const long long g = iscr[0];
     if (g >= n_groups) break;
-    const long long base = (g * Q + q) * kS1Group;   // first source of this team
+    const long long base = (g * Q + q) * G;   // first source of this team
     // ---- phase 1: parameters and centre roots of source base + t --------------------------------------------------
     {
       const long long src = base + t;
-      if (src < n) {
+      if (t < G && src < n) {
         const SourceParams S = load_source(p.b, src);
         prm[0 * kS1Group + t] = S.L.s;
         prm[1 * kS1Group + t] = S.L.m1;
@@ -106,9 +108,9 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
     }
     __syncthreads();
     // ---- phase 2: one source per team at a time, one thread per boundary sample ---------------------------------------
-    const int cnt = (int)((n - base < kS1Group) ? (n > base ? n - base : 0) : kS1Group);   // of this team
-    for (int i = 0; i < kS1Group; ++i) {
-      if (g * Q * kS1Group + i >= n) break;              // CTA-uniform: no team has a source i
+    const int cnt = (int)((n - base < G) ? (n > base ? n - base : 0) : G);   // of this team
+    for (int i = 0; i < G; ++i) {
+      if (g * Q * G + i >= n) break;              // CTA-uniform: no team has a source i
       const int code = (i < cnt) ? (int)prm[7 * kS1Group + i] : 0;
       const bool active = (code & 256) != 0;            // team-uniform
       double rho = 1.0;
@@ -176,7 +178,7 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
 #pragma unroll
       for (int qq = 0; qq < Q; ++qq) {
         const double Aq = sc[qq * 4] + sc[qq * 4 + 2], Eq = sc[qq * 4 + 1] + sc[qq * 4 + 3];
-        const bool act = ((g * Q + qq) * kS1Group + i < n) && (((int)prm_all[(qq * kS1ParamRows + 7) * kS1Group + i]) & 256);
+        const bool act = ((g * Q + qq) * G + i < n) && (((int)prm_all[(qq * kS1ParamRows + 7) * kS1Group + i]) & 256);
         const bool fin = isfinite(Aq) && isfinite(Eq);
         const bool pd = act && fin && !(Eq <= p.tol * fabs(Aq)) && !p.final_stage;   // stop rule P:272
         any_pend = any_pend || pd;
@@ -237,7 +239,7 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
     // ---- phase 3: coalesced results -----------------------------------------------------------------------------------
     {
       const long long src = base + t;
-      if (src < n && !res_pend[t]) {
+      if (t < G && src < n && !res_pend[t]) {
         p.out_mu[src] = res_mu[t];
         if (p.out_err) p.out_err[src] = res_err[t];
         if (p.out_nsamples) p.out_nsamples[src] = res_ns[t];
