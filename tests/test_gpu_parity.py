@@ -156,6 +156,23 @@ def test_full_size_config3_sampled_outputs(ctx):
     assert np.median(rel) < 1e-5
 
 
+@pytest.mark.parametrize("name,kw", [("fig5_map", dict(case="close")), ("fig5_map", dict(case="resonant")),
+                                     ("fig5_map", dict(case="wide")), ("fig7_grid", {}), ("lowq_sweep", {})])
+def test_adaptive_paper_workloads(ctx, name, kw):
+    """the paper's own caustic-dense inputs -- the three 480 x 340 source-plane maps of Fig. 5
+    (P:342), the (s, q) sweep of Fig. 7 with 30 x 30 sources per lens over the caustic, and a low-q
+    sweep over the validated domain 0.1 <= s <= 10, q >= 1e-9.  Same bars as the BASELINE configs."""
+    full = W.get(name, **kw)
+    wl = _subsample(full, min(1500, full.n_sources), 11)
+    check_adaptive_like_for_like(ctx, wl, 1e-4)
+    g, _ = check_adaptive_acceptance(ctx, wl)
+    # the whole workload in one call at its own tolerance: every output finite, converged, never below 1
+    r = ctx.magnify_workload(full, 1e-4)
+    st = r["status"].astype(np.uint32)
+    assert np.all(np.isfinite(r["mu"])) and np.all(r["mu"] >= 1.0 - 1e-6) and np.all(st & 3)
+    assert (st & 1).mean() > 0.999
+
+
 def test_handover_and_recompute_paths_agree():
     """Stage 1 hands the first iteration of an unfinished source to stage 2 through the hand-over arena; without a
     free slot stage 2 recomputes it.  Same arithmetic either way (up to the compiler's contraction choices in the

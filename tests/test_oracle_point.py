@@ -189,3 +189,22 @@ def test_double_and_long_double_classify_alike():
         assert sorted(ia) == [0, 1, 2, 3, 4]
         assert np.all(a["kind"][ia] == b["kind"])
         assert np.abs(a["z"][ia] - b["z"]).max() < 1e-9
+
+
+def test_paper_workload_generators_shapes():
+    """SURVEY 8(f) N2/N3 inputs: shapes and placement as documented (Fig. 5: 480 x 340 maps centred on the origins
+    the caption prints; Fig. 7: 30 x 30 sources per lens; low-q sweep inside P:374's domain)."""
+    import workloads as W
+    m = W.fig5_map("close")
+    assert m.n_sources == 480 * 340 and m.n_models == 1 and m.rho[0] == 5e-5
+    assert abs(m.zeta[:, 0].mean() + 1.5) < 1e-12 and abs(m.zeta[:, 1].mean() - 0.035) < 1e-12
+    assert abs(W.fig5_map("wide").zeta[:, 0].mean() - 2.666) < 1e-12
+    g = W.fig7_grid()
+    assert g.n_sources == g.n_models * 900 and g.s.min() == 0.5 and g.s.max() == 3.0
+    assert abs(g.q.min() - 1e-6) < 1e-18 and abs(g.q.max() - 1e-2) < 1e-12 and np.all(g.rho == 1e-4)
+    lo = W.lowq_sweep()
+    assert lo.q.min() >= 1e-9 and lo.q.max() <= 1e-6 and lo.s.min() >= 0.1 and lo.s.max() <= 10.0
+    # the oracle finds caustic crossings in a sample of the low-q sweep (the placement does its job)
+    sub = lo.subset(np.arange(0, lo.n_sources, 40))
+    r = api.magnify(sub, 1e-4, mode=0)
+    assert (r["nsamples"] > 64).mean() > 0.05 and np.all(r["status"] & 1)

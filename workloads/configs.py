@@ -140,7 +140,76 @@ def fig6_case(n: int = 201, half_width: float = 4e-4) -> Workload:
     return _single_model("fig6", 0.5, 1e-6, 1e-4, xs - 0.0035j, 1e-4)
 
 
+# ---------------------------------------------------------------------------------------------------------
+# Second workload family: the paper's own caustic-dense test inputs.  Window extents are
+# figure-only in the paper (not in its text); the ones below are this repo's choice and are stated here.
+# ---------------------------------------------------------------------------------------------------------
+_FIG5 = {
+    # name: (s, q, rho, origin of the map = position of the planetary / resonant caustic, half-width in x)
+    "close": (0.5, 1e-4, 5e-5, -1.5 + 0.035j, 4e-3),
+    "resonant": (1.0, 1e-4, 1e-3, 0.0 + 0.0j, 0.12),
+    "wide": (3.0, 1e-4, 1e-4, 2.666 + 0.0j, 8e-3),
+}
+
+
+def fig5_map(case: str = "close", nx: int = 480, ny: int = 340) -> Workload:
+    """PAPER.md:342, P:352 (Fig. 5): source-plane map of nx x ny = 480 x 340 extended sources over the planetary
+    (s = 0.5, 3) or resonant (s = 1) caustic, q = 1e-4, rho matched to the caustic, tol 1e-4.  Cell-centred grid,
+    row-major with y outer, centred on the origin the caption gives; half-width in x as tabulated above (about twice
+    the caustic), half-width in y = half-width in x * ny / nx."""
+    s, q, rho, o, hx = _FIG5[case]
+    hy = hx * ny / nx
+    x = o.real - hx + 2.0 * hx * (np.arange(nx) + 0.5) / nx
+    y = o.imag - hy + 2.0 * hy * (np.arange(ny) + 0.5) / ny
+    return _single_model("fig5_" + case, s, q, rho, x[None, :] + 1j * y[:, None], 1e-4, nx=nx, ny=ny)
+
+
+def _planetary_caustic(s, q):
+    """Centre and linear scale of the planetary caustic (textbook perturbative expressions, used only to PLACE
+    source grids): on the axis at s - 1/s for wide binaries, off the axis by 2 sqrt(q (1 - s^2)) / s for close ones;
+    scale ~ sqrt(q) s^3 (close), sqrt(q) / s^2 (wide), never more than the resonant size ~ q^(1/3)."""
+    xc = s - 1.0 / s
+    yc = np.where(s < 1.0, 2.0 * np.sqrt(q * np.maximum(1.0 - s * s, 0.0)) / s, 0.0)
+    scale = np.where(s < 1.0, np.sqrt(q) * s ** 3, np.sqrt(q) / s ** 2)
+    return xc + 1j * yc, np.minimum(4.0 * scale, 1.5 * q ** (1.0 / 3.0))
+
+
+def fig7_grid(n_s: int = 16, n_q: int = 12, n_side: int = 30, rho: float = 1e-4) -> Workload:
+    """PAPER.md:368 (Fig. 7): parameter-space sweep.  n_s x n_q lenses, s linear in [0.5, 3], q log-spaced in
+    [1e-6, 1e-2]; each with an n_side x n_side = 30 x 30 cell-centred grid of sources of radius rho = 1e-4 covering
+    the planetary (resonant) caustic: centred on it, half-width max(2 x caustic scale, 10 rho).  tol 1e-4."""
+    sv = np.linspace(0.5, 3.0, n_s)
+    qv = np.exp(np.linspace(np.log(1e-6), np.log(1e-2), n_q))
+    S, Q = [a.ravel() for a in np.meshgrid(sv, qv, indexing="ij")]
+    c, scale = _planetary_caustic(S, Q)
+    hw = np.maximum(2.0 * scale, 10.0 * rho)
+    u = -1.0 + 2.0 * (np.arange(n_side) + 0.5) / n_side
+    g = (u[None, :] + 1j * u[:, None]).ravel()                          # [n_side^2]
+    zc = c[:, None] + hw[:, None] * g[None, :]
+    n_m = S.size
+    model_id = np.repeat(np.arange(n_m, dtype=np.int32), n_side * n_side)
+    return Workload("fig7_grid", _f64(S), _f64(Q), _f64(np.full(n_m, rho)), np.ascontiguousarray(model_id), _pack(zc),
+                    1e-4, meta={"n_s": n_s, "n_q": n_q, "n_side": n_side})
+
+
+def lowq_sweep(n: int = 4000, seed: int = 250103324) -> Workload:
+    """Low-mass-ratio robustness sweep over the validated domain of P:374 (0.1 <= s <= 10, q >= 1e-9): n sources,
+    each with its own lens: s log-uniform in [0.1, 10], q log-uniform in [1e-9, 1e-6], rho log-uniform in
+    [1e-4, 1e-2]; the source centre is drawn uniformly in a square of half-width 3 max(rho, caustic scale) around
+    the planetary caustic, so most disks touch or cover it.  tol 1e-4."""
+    rng = np.random.default_rng(seed)
+    s = np.exp(rng.uniform(np.log(0.1), np.log(10.0), n))
+    q = np.exp(rng.uniform(np.log(1e-9), np.log(1e-6), n))
+    rho = np.exp(rng.uniform(np.log(1e-4), np.log(1e-2), n))
+    c, scale = _planetary_caustic(s, q)
+    hw = 3.0 * np.maximum(rho, scale)
+    zc = c + hw * (rng.uniform(-1.0, 1.0, n) + 1j * rng.uniform(-1.0, 1.0, n))
+    return Workload("lowq_sweep", _f64(s), _f64(q), _f64(rho), np.arange(n, dtype=np.int32), _pack(zc), 1e-4,
+                    meta={"seed": seed})
+
+
 def get(name: str, **kw) -> Workload:
     table = {"config1": config1, "config2": config2, "config3": config3, "config4": config4,
-             "config5": config5, "fig1": fig1_case, "fig2": fig2_case, "fig6": fig6_case}
+             "config5": config5, "fig1": fig1_case, "fig2": fig2_case, "fig6": fig6_case, "fig5_map": fig5_map,
+             "fig7_grid": fig7_grid, "lowq_sweep": lowq_sweep}
     return table[name](**kw)
