@@ -43,6 +43,8 @@ extern "C" {
                              /* non-finite / non-positive s, q, rho or non-finite zeta: out_mu = NaN             */
 #define TWK_ST_NUMERIC 16u   /* a non-finite value appeared in the solve (degenerate quintic, zeta on a lens)    */
 #define TWK_ST_SLOPE 32u     /* the slope detector re-judged a real image pair as ghosts (reading G-4) */
+#define TWK_ST_POINT 64u     /* point-source adequacy tests passed: out_mu = point-source magnification +   */
+                             /* quadrupole term, no contour was integrated, out_nsamples = 0                        */
 
 typedef struct twk_ctx twk_ctx; /* opaque; owns only its device scratch workspace */
 
@@ -63,6 +65,11 @@ typedef struct {
                         /* 0 switches the detector off.  Adaptive mode only.                                           */
   double slope_cos;     /* largest |cos| of the angle between the two pairs still counted as perpendicular; default    */
                         /* cos 45 deg (reading G-4).  0 <= slope_cos <= 1.                                             */
+  int point_source_test; /* 1 = before the contour integration, test whether the point-source magnification plus its   */
+                        /* quadrupole (finite-source) term is accurate to rel_tol: quadrupole test + ghost-image test  */
+                        /* (formulas derived in DESIGN.md, readings N1-a..c).  Sources that pass get that value  */
+                        /* (status TWK_ST_POINT, out_err = relative size of the quadrupole term, out_nsamples = 0) and  */
+                        /* skip the contour.  Default 0: every source takes the contour path.                           */
 } twk_options;
 
 /* Fill *opt with the defaults above. */

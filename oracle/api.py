@@ -29,6 +29,7 @@ def lib():
                                        _D, _I8, _I8, _D, _D, _I32, _D]
         L.orc_magnify.argtypes = [C.c_int64, _D, _D, _D, C.c_int64, _I32, _D, C.c_double, C.c_int, C.c_int, C.c_int,
                                   C.c_int, C.c_int, C.c_int, C.c_int, _D, _D, _I32, _U32, C.c_double, C.c_double]
+        L.orc_point_source.argtypes = [C.c_int64, _D, _D, _D, C.c_int64, _I32, _D, C.c_double, C.c_int, _I8, _D, _D, _D]
         L.orc_magnify_thetas.argtypes = [C.c_double] * 6 + [C.c_int] * 5 + [_D]
         L.orc_magnify_thetas.restype = C.c_int
         L.orc_rayshoot.argtypes = [C.c_double] * 9 + [C.c_int] * 4
@@ -117,6 +118,19 @@ def magnify(wl, rel_tol=None, mode=0, prec=0, nthreads=0, samples_per_iter=64, i
                       initial_samples, max_samples, subtract_avg_tol, prec, nthreads, _p(mu, _D), _p(err, _D), _p(ns, _I32),
                       _p(st, _U32), float(slope_gate), float(slope_cos))
     return dict(mu=mu, err=err, nsamples=ns, status=st)
+
+
+def point_source(wl, rel_tol=None, prec=0):
+    """N1: point-source adequacy tests over a Workload.  Returns dict(accept bool[n], mu = point source +
+    quadrupole term, qrel = relative size of the quadrupole term, A = point-source magnification)."""
+    s, q, rho, mid, zeta = _batch(wl)
+    n = zeta.shape[0]
+    tol = float(wl.rel_tol if rel_tol is None else rel_tol)
+    acc = np.zeros(n, np.int8)
+    mu, qrel, A = np.zeros(n), np.zeros(n), np.zeros(n)
+    lib().orc_point_source(len(s), _p(s, _D), _p(q, _D), _p(rho, _D), n, _p(mid, _I32), _p(zeta, _D), tol, prec, _p(acc, _I8),
+                           _p(mu, _D), _p(qrel, _D), _p(A, _D))
+    return dict(accept=acc.astype(bool), mu=mu, qrel=qrel, A=A)
 
 
 def magnify_thetas(s, q, rho, zeta_c, rel_tol, prec=0, samples_per_iter=64, initial_samples=64, max_samples=4096,

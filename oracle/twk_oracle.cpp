@@ -607,6 +607,78 @@ void magnify_one(double s, double q, double rho_, double zre, double zim, double
     for (size_t i = 0; i < C.S.size() && (int)i < o.max_samples; ++i) out_theta[i] = (double)C.S[i].theta;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// N1: point-source adequacy tests, P:122 ("the quadrupole test and ghost image test check if the
+// point-source approximation is accurate enough").  The paper prints no formulas; readings N1-a..c derive
+// them from the lens equation:
+//   N1-a  uniform disk: mu_fs = mu + (rho^2/8) Lap(mu) + O(rho^4), Lap = 4 d2/(dzeta dzetabar).  For one image, with
+//         g, h, k the first three derivatives of f at the image and J = 1 - |g|^2: any F(z, zbar) has
+//         dF/dzeta = (F_z - g F_zb)/J and dF/dzetabar = (F_zb - gbar F_z)/J (from dz/dzeta = 1/J, dz/dzetabar = -gbar/J).
+//         Applied twice to F = 1/J.
+//   N1-b  quadrupole test: sum_real rho^2/2 (|d2(1/J)/(dzeta dzetabar)| + |d2(1/J)/dzeta^2|) < c_Q * tol * A,  c_Q = 3.
+//         The second, traceless derivative does not enter the disk average, but next to a cusp the Laplacian of a
+//         bright image changes sign while the traceless part stays large: bounding both keeps the next order small.
+//   N1-c  ghost-image test: a ghost root responds to a source shift delta by (delta - f'(w) conj(delta)) / (1 - f'(w) f'(z)),
+//         w = conj(zeta) - f(z) (differentiate the 2-cycle); the pair becomes real when it closes its separation |R|:
+//         rho (1 + |f'(w)|) / |1 - f'(w) f'(z)| < c_G |R|,  c_G = 0.1
+// ---------------------------------------------------------------------------------------------------------
+template <class R>
+struct PsOut { int accept; R mu, qrel, A; int nreal; };
+
+template <class R>
+PsOut<R> point_source_test(double s, double q, double rho_, double zre, double zim, double tol) {
+  const Lens<R> L = make_lens<R>(s, q);
+  const R rho = (R)rho_;
+  Sample<R> S;
+  // the point source at the centre: theta is irrelevant for the images; rho = 0 puts the sample on the centre
+  point_solve(L, Cx<R>((R)zre, (R)zim), R(0), R(0), S);
+  const Cx<R> zeta((R)zre, (R)zim);
+  const R z1 = L.z1, z2 = L.z2;                  // CM frame lens positions, Eq.(2)
+  PsOut<R> o;
+  o.accept = 1;
+  o.nreal = S.nreal;
+  R A = 0, Q = 0, Qabs = 0;
+  for (int k = 0; k < 5; ++k) {
+    const Cx<R> z = S.z[k];
+    const Cx<R> a = R(1) / (z1 - z), b = R(1) / (z2 - z);
+    const Cx<R> f = L.m1 * a + L.m2 * b;
+    const Cx<R> g = L.m1 * a * a + L.m2 * b * b;
+    if (S.kind[k] == 0) {   // N1-c
+      const Cx<R> w = std::conj(zeta) - f;
+      const Cx<R> aw = R(1) / (z1 - w), bw = R(1) / (z2 - w);
+      const Cx<R> gw = L.m1 * aw * aw + L.m2 * bw * bw;
+      const R resp = (R(1) + std::abs(gw)) / std::abs(Cx<R>(1, 0) - gw * g);
+      if (!(rho * resp < R(0.1) * std::abs(S.Res[k]))) o.accept = 0;
+      continue;
+    }
+    const Cx<R> h = R(2) * (L.m1 * a * a * a + L.m2 * b * b * b);
+    const Cx<R> kk = R(6) * (L.m1 * a * a * a * a + L.m2 * b * b * b * b);
+    const R J = R(1) - std::norm(g);
+    // F = 1/J:  F_z = -J_z / J^2,  J_z = -h conj(g),  J_zb = -g conj(h)
+    // first derivative  M = dF/dzeta = N / J^3,  N = h conj(g) - g^2 conj(h)
+    const Cx<R> N = h * std::conj(g) - g * g * std::conj(h);
+    const Cx<R> Nz = kk * std::conj(g) - R(2) * g * h * std::conj(h);
+    const Cx<R> Nzb = h * std::conj(h) - g * g * std::conj(kk);
+    const Cx<R> Jz = -h * std::conj(g), Jzb = -g * std::conj(h);
+    const R J3 = J * J * J, J4 = J3 * J;
+    const Cx<R> Mz = Nz / J3 - R(3) * N * Jz / J4;
+    const Cx<R> Mzb = Nzb / J3 - R(3) * N * Jzb / J4;
+    const Cx<R> d2 = (Mzb - std::conj(g) * Mz) / J;           // d2(1/J) / (dzeta dzetabar)
+    const R p = (J > 0) ? R(1) : R(-1);
+    A += p / J;
+    Q += p * R(0.5) * rho * rho * d2.real();
+    const Cx<R> t2 = (Mz - g * Mzb) / J;                       // d2(1/J) / dzeta^2, the traceless part
+    Qabs += R(0.5) * rho * rho * (std::abs(d2) + std::abs(t2));
+  }
+  if (S.repaired) o.accept = 0;                                 // leave noise-floor cases to the contour
+  o.A = A;
+  o.mu = A + Q;
+  o.qrel = Qabs / std::abs(A);
+  if (!(Qabs < R(3) * (R)tol * std::abs(A))) o.accept = 0;      // N1-b
+  if (!std::isfinite((double)o.mu) || !std::isfinite((double)o.qrel)) o.accept = 0;
+  return o;
+}
+
 template <class R>
 void point_out(double s, double q, double rho, double zre, double zim, double theta, double* z, double* Res,
                       double* J, int32_t* kind, double* zp, double* w, int32_t* info) {
@@ -726,6 +798,30 @@ void orc_magnify(int64_t n_models, const double* s, const double* q, const doubl
       magnify_one<double>(s[m], q[m], rho[m], zeta[2 * i], zeta[2 * i + 1], rel_tol, mode, o, out_mu ? out_mu + i : nullptr,
                           out_err ? out_err + i : nullptr, out_nsamples ? out_nsamples + i : nullptr,
                           out_status ? out_status + i : nullptr, nullptr);
+  }
+}
+
+// N1: point-source adequacy tests over a batch.  out_accept[i] in {0,1}; out_mu = point source + quadrupole term;
+// out_qrel = relative size of the quadrupole term; out_A = point-source magnification (sum of 1/|J| over real images).
+void orc_point_source(int64_t n_models, const double* s, const double* q, const double* rho, int64_t n_sources,
+                      const int32_t* model_id, const double* zeta, double rel_tol, int prec, int8_t* out_accept,
+                      double* out_mu, double* out_qrel, double* out_A) {
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t i = 0; i < n_sources; ++i) {
+    const int64_t m = model_id ? model_id[i] : (n_models == 1 ? 0 : i);
+    int acc;
+    double mu, qr, A;
+    if (prec) {
+      const auto o = point_source_test<long double>(s[m], q[m], rho[m], zeta[2 * i], zeta[2 * i + 1], rel_tol);
+      acc = o.accept; mu = (double)o.mu; qr = (double)o.qrel; A = (double)o.A;
+    } else {
+      const auto o = point_source_test<double>(s[m], q[m], rho[m], zeta[2 * i], zeta[2 * i + 1], rel_tol);
+      acc = o.accept; mu = o.mu; qr = o.qrel; A = o.A;
+    }
+    if (out_accept) out_accept[i] = (int8_t)acc;
+    if (out_mu) out_mu[i] = mu;
+    if (out_qrel) out_qrel[i] = qr;
+    if (out_A) out_A[i] = A;
   }
 }
 

@@ -2,8 +2,8 @@
 (the hot path of arXiv 2501.03322, "Twinkle").  The product is csrc/ (CUDA, sm_100a) behind the C ABI of
 include/twk.h; this package is the thin Python binding (argument marshalling only).  There is no CPU fallback:
 every compute entry point raises if libtwk.so or a CUDA device is missing."""
-from .binding import (TWK_ST_CAP, TWK_ST_CONVERGED, TWK_ST_DOMAIN, TWK_ST_NUMERIC, TWK_ST_REPAIRED, TWK_ST_SLOPE, Context, TwkError,
+from .binding import (TWK_ST_CAP, TWK_ST_CONVERGED, TWK_ST_DOMAIN, TWK_ST_NUMERIC, TWK_ST_POINT, TWK_ST_REPAIRED, TWK_ST_SLOPE, Context, TwkError,
                       exported_symbols, lib, library_path, twk_fp64_peak_probe, twk_version, twk_workspace_bytes)
 
 __all__ = ["Context", "TwkError", "lib", "library_path", "exported_symbols", "twk_workspace_bytes", "twk_version",
-           "twk_fp64_peak_probe", "TWK_ST_CONVERGED", "TWK_ST_CAP", "TWK_ST_REPAIRED", "TWK_ST_DOMAIN", "TWK_ST_NUMERIC", "TWK_ST_SLOPE"]
+           "twk_fp64_peak_probe", "TWK_ST_CONVERGED", "TWK_ST_CAP", "TWK_ST_REPAIRED", "TWK_ST_DOMAIN", "TWK_ST_NUMERIC", "TWK_ST_SLOPE", "TWK_ST_POINT"]

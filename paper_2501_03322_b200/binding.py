@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(HERE, "libtwk.so")
 _lib = None
 
-TWK_ST_CONVERGED, TWK_ST_CAP, TWK_ST_REPAIRED, TWK_ST_DOMAIN, TWK_ST_NUMERIC, TWK_ST_SLOPE = 1, 2, 4, 8, 16, 32
+TWK_ST_CONVERGED, TWK_ST_CAP, TWK_ST_REPAIRED, TWK_ST_DOMAIN, TWK_ST_NUMERIC, TWK_ST_SLOPE, TWK_ST_POINT = 1, 2, 4, 8, 16, 32, 64
 
 SYMBOLS = ["twk_default_options", "twk_create", "twk_destroy", "twk_workspace_bytes", "twk_magnify", "twk_images_fixed",
            "twk_magnify_host", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_strerror", "twk_version"]
@@ -26,7 +26,7 @@ class TwkError(RuntimeError):
 
 class twk_options(C.Structure):
     _fields_ = [("samples_per_iter", C.c_int), ("initial_samples", C.c_int), ("max_samples", C.c_int),
-                ("subtract_avg_tol", C.c_int), ("handoff_slots", C.c_int64), ("slope_gate", C.c_double), ("slope_cos", C.c_double)]
+                ("subtract_avg_tol", C.c_int), ("handoff_slots", C.c_int64), ("slope_gate", C.c_double), ("slope_cos", C.c_double), ("point_source_test", C.c_int)]
 
 
 def library_path() -> str:

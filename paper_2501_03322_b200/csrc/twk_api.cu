@@ -66,7 +66,8 @@ Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
 
 bool valid_options(const twk_options& o) {
   return o.samples_per_iter == twk::kThreads && o.initial_samples == twk::kThreads && o.max_samples >= twk::kThreads &&
-         o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1) && o.handoff_slots >= -1 && o.slope_gate >= 0.0 && o.slope_cos >= 0.0 && o.slope_cos <= 1.0;
+         o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1) && o.handoff_slots >= -1 && o.slope_gate >= 0.0 && o.slope_cos >= 0.0 && o.slope_cos <= 1.0 &&
+         (o.point_source_test == 0 || o.point_source_test == 1);
 }
 
 int cuda_fail(cudaError_t e) {
@@ -135,6 +136,7 @@ void twk_default_options(twk_options* opt) {
   opt->handoff_slots = -1;
   opt->slope_gate = 1e-5;
   opt->slope_cos = 0.70710678118654752;
+  opt->point_source_test = 0;
 }
 
 size_t twk_workspace_bytes(const twk_options* opt, size_t max_sources) {
@@ -246,6 +248,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
     twk::Stage1Args a1{};
     a1.b = a.b;
     a1.tol = rel_tol;
+    a1.ps_test = ctx->opt.point_source_test;
     a1.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
     a1.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
     a1.final_stage = P.cap2 ? 0 : 1;

@@ -233,6 +233,116 @@ TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int st
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// N1: point-source adequacy tests in front of the contour path ("the quadrupole test and ghost
+// image test check if the point-source approximation is accurate enough").  The paper gives no formulas; these are
+// derived here (readings N1-a..c) from the lens equation alone:
+//  * a uniform disk of radius rho sees  mu_fs = mu + (rho^2 / 8) Laplacian(mu) + O(rho^4),  Laplacian = 4 d^2/dzeta dzetabar;
+//    for one image with g = f1(z), h = f2(z), k = f3(z) (first, second, third derivative of f), J = 1 - g gbar, the
+//    chain rule through dz/dzeta = 1/J, dz/dzetabar = -gbar/J gives  d(1/J)/dzeta = N / J^3,  N = h gbar - g^2 hbar,
+//    and  d^2(1/J)/dzeta dzetabar = [ -gbar (N_z/J^3 - 3 N J_z/J^4) + (N_zb/J^3 - 3 N J_zb/J^4) ] / J  with
+//    N_z = k gbar - 2 g h hbar, N_zb = h hbar - g^2 kbar, J_z = -h gbar, J_zb = -g hbar;
+//    the same operator once more in zeta gives the traceless second derivative d^2(1/J)/dzeta^2 = (M_z - g M_zb)/J,
+//    M = N/J^3.  The disk average keeps only the Laplacian, but next to a cusp the Laplacian of a bright image
+//    changes sign while the traceless part stays large, so the test bounds both;
+//  * quadrupole test: sum over real images of rho^2/2 (|d2/dzeta dzetabar| + |d2/dzeta^2|) of 1/J < kPsQuad * tol * A;
+//  * ghost-image test: a ghost root moves by A_k delta + B_k conj(delta) (centre_seeds); the pair merges into a real
+//    pair when the two close their separation |R_k| (the 2-cycle step): require rho (|A_k| + |B_k|) < kPsGhost |R_k|.
+// Returns true when both tests pass; mu = A + quadrupole term, qrel = the size of the quadrupole term relative to A.
+// ------------------------------------------------------------------------------------------------------------
+constexpr double kPsQuad = 3.0;    // reading N1-b: calibrated against the converged contour values of the oracle
+constexpr double kPsGhost = 0.1;   // reading N1-c
+
+TWK_HD bool point_source_adequate(const Lens& L, cd zc, double rho, const double* seeds, int stride, double tol, double& mu,
+                                  double& qrel) {
+  const cd y = mk(zc.x - L.z2, zc.y);
+  cd eta[5], g[5], f[5], Res[5];
+  double R2[5];
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    eta[k] = mk(seeds[k * stride], seeds[(5 + k) * stride]);
+    const cd a = crecip(mk(-L.s - eta[k].x, -eta[k].y));
+    const cd b = crecip(-eta[k]);
+    f[k] = L.m1 * a + L.m2 * b;
+    g[k] = L.m1 * (a * a) + L.m2 * (b * b);
+    Res[k] = mk(y.x - eta[k].x - f[k].x, y.y - eta[k].y + f[k].y);
+    R2[k] = norm2(Res[k]);
+  }
+  // residual detector, as in point_solve_cs
+  int ia = 0;
+#pragma unroll
+  for (int k = 1; k < 5; ++k)
+    if (R2[k] > R2[ia]) ia = k;
+  int ib = (ia == 0) ? 1 : 0;
+#pragma unroll
+  for (int k = 0; k < 5; ++k)
+    if (k != ia && R2[k] > R2[ib]) ib = k;
+  cd eA = eta[0], eB = eta[0], rA = Res[0], rB = Res[0];
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    if (k == ia) { eA = eta[k]; rA = Res[k]; }
+    if (k == ib) { eB = eta[k]; rB = Res[k]; }
+  }
+  const cd dab = eB - eA;
+  const bool ghost = norm2(rA - dab) < norm2(rA) && norm2(rB + dab) < norm2(rB);
+  double A = 0.0, Q = 0.0, Qabs = 0.0;
+  int npos = 0, nreal = 0;
+  bool ok = true;
+  const double hr2 = 0.5 * rho * rho;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const cd a = crecip(mk(-L.s - eta[k].x, -eta[k].y));
+    const cd b = crecip(-eta[k]);
+    const cd a2 = a * a, b2 = b * b;
+    if (ghost && (k == ia || k == ib)) {
+      // ghost-image test: response of the ghost root, A = 1/D, B = -f1(w)/D, D = 1 - f1(w) f1(z), w = conj(y) - f(z)
+      const cd w = mk(y.x - f[k].x, -y.y - f[k].y);
+      const cd aw = crecip(mk(-L.s - w.x, -w.y));
+      const cd bw = crecip(-w);
+      const cd gw = L.m1 * (aw * aw) + L.m2 * (bw * bw);
+      const cd D = mk(1.0, 0.0) - gw * g[k];
+      const double resp = (1.0 + sqrt(norm2(gw))) * sqrt(rcp(norm2(D)));   // |A| + |B|
+      ok = ok && (rho * resp < kPsGhost * sqrt(R2[k]));
+      continue;
+    }
+    const cd h = 2.0 * (L.m1 * (a2 * a) + L.m2 * (b2 * b));
+    const cd kk = 6.0 * (L.m1 * (a2 * a2) + L.m2 * (b2 * b2));
+    const cd gb = conj(g[k]), hb = conj(h), kb = conj(kk);
+    const double J = 1.0 - norm2(g[k]);
+    const double iJ = rcp(J), iJ3 = iJ * iJ * iJ, iJ4 = iJ3 * iJ;
+    const cd g2 = g[k] * g[k];
+    const cd N = h * gb - g2 * hb;
+    const cd Nz = kk * gb - 2.0 * ((g[k] * h) * hb);
+    const cd Nzb = h * hb - g2 * kb;
+    const cd Jz = -(h * gb), Jzb = -(g[k] * hb);
+    const cd Mz = iJ3 * Nz - (3.0 * iJ4) * (N * Jz);
+    const cd Mzb = iJ3 * Nzb - (3.0 * iJ4) * (N * Jzb);
+    const cd mzz = iJ * (Mzb - gb * Mz);                  // d2(1/J) / dzeta dzetabar  (a quarter of the Laplacian)
+    const cd mz2 = iJ * (Mz - g[k] * Mzb);                // d2(1/J) / dzeta^2         (the traceless part)
+    const double p = (J > 0.0) ? 1.0 : -1.0;
+    A += p * iJ;
+    Q += p * hr2 * mzz.x;
+    Qabs += hr2 * (sqrt(norm2(mzz)) + sqrt(norm2(mz2)));
+    npos += (J > 0.0);
+    ++nreal;
+  }
+  ok = ok && (npos == ((nreal - 1) >> 1));             // parity sum -1; no repair here: leave it to the contour
+  mu = A + Q;
+  qrel = Qabs * rcp(fabs(A));
+  return ok && isfinite(mu) && isfinite(qrel) && (Qabs < kPsQuad * tol * fabs(A));
+}
+
+// out-of-line entry (once per source, outside the hot loop: keeps its registers and code away from it)
+struct PsResult {
+  double mu, qrel;
+  int ok;
+};
+TWK_NOINLINE PsResult point_source_adequate_cold(Lens L, cd zc, double rho, const double* seeds, int stride, double tol) {
+  PsResult r;
+  r.ok = point_source_adequate(L, zc, rho, seeds, stride, tol, r.mu, r.qrel) ? 1 : 0;
+  return r;
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // a6 + a7: one interval theta_A -> theta_B (dth = theta_B - theta_A > 0).
 // ------------------------------------------------------------------------------------------------------------
 struct Piece {

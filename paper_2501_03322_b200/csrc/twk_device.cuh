@@ -271,6 +271,10 @@ TWK_NOINLINE Roots5 quintic_roots_cold(Coef6 C) {
 // are polished by the same Newton sweeps and the verification is repeated.
 // Returns false when that fails too; the caller then falls back to the cold solver quintic_roots().
 // r[] holds the seeds on entry and the roots on exit.
+// Two converged chains are the same root when they agree to 1e-6 of their size (RELATIVE: next to a planet of
+// q = 1e-9 two distinct roots can be 1e-9 apart in absolute terms while the other roots are of order one).
+constexpr double kDupRel2 = 1e-12;
+
 struct SeededState {
   cd r[5];
   unsigned done;
@@ -281,14 +285,14 @@ struct SeededState {
 TWK_NOINLINE SeededState seeded_recover(cd c0, cd c5, cd tot, SeededState S) {
   TWK_COUNT(recovery);
   cd (&r)[5] = S.r;
-  const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
   // good = converged and not a duplicate of an earlier good root
   unsigned good = S.done;
 #pragma unroll
   for (int a = 0; a < 5; ++a)
 #pragma unroll
     for (int b = a + 1; b < 5; ++b)
-      if ((good >> a & 1u) && (good >> b & 1u) && norm2(r[a] - r[b]) <= 1e-18 * scale * scale) good &= ~(1u << b);
+      if ((good >> a & 1u) && (good >> b & 1u) && norm2(r[a] - r[b]) <= kDupRel2 * (norm2(r[a]) + norm2(r[b])))
+        good &= ~(1u << b);
   int ng = 0;
 #pragma unroll
   for (int k = 0; k < 5; ++k) ng += (good >> k) & 1u;
@@ -367,8 +371,15 @@ TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5]) {
   bool recovered = false;
   for (int it = 2; it < 22; ++it) {
     if (done == 31u || (it >= 10 && !recovered)) {
-      const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
-      if (done == 31u && abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale) return true;
+      if (done == 31u) {
+        // verification by Vieta: the sum of the roots (absolute, on the scale of the largest) and their product
+        // (relative: two chains on one of two tiny neighbouring roots next to a q = 1e-9 planet change the sum by
+        // 1e-9 of its scale but the product by their relative distance)
+        const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
+        const cd prod = ((r[0] * r[1]) * (r[2] * r[3])) * r[4];
+        const cd dp = prod * c[5] + c[0];                 // prod = -c0/c5
+        if (abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale && abs1(dp) <= 1e-9 * abs1(c[0])) return true;
+      }
       if (recovered) break;
       recovered = true;
       SeededState S;

@@ -22,6 +22,7 @@ struct Stage1Args {
   double tol;
   double slope_gate2;    // square of the slope detector's proximity gate (twk_options.slope_gate)
   double slope_cos2;     // square of the largest |cos| still counted as perpendicular (twk_options.slope_cos)
+  int ps_test;           // N1: point-source adequacy tests in front of the contour path (twk_options.point_source_test)
   int group;             // sources per group, 1..64 (smaller for small batches: more CTAs get work)
   int final_stage;       // 1: there is no refinement stage (max_samples < 128): cap status instead of pending
   int* cursor;           // group fetch counter (zeroed before launch)
@@ -102,8 +103,22 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
         prm[4 * kS1Group + t] = S.zc.x;
         prm[5 * kS1Group + t] = S.zc.y;
         prm[6 * kS1Group + t] = S.rho;
-        prm[7 * kS1Group + t] = double((int)S.status | (S.valid ? 256 : 0));
-        if (S.valid) centre_seeds(S.L, S.zc, S.rho, seeds + t, kS1Group);
+        int code = (int)S.status | (S.valid ? 256 : 0);
+        if (S.valid) {
+          centre_seeds(S.L, S.zc, S.rho, seeds + t, kS1Group);
+          if (p.ps_test) {   // N1: quadrupole + ghost-image tests; adequate -> no contour for this source
+            const PsResult r = point_source_adequate_cold(S.L, S.zc, S.rho, seeds + t, kS1Group, p.tol);
+            if (r.ok) {
+              res_mu[t] = r.mu;
+              res_err[t] = r.qrel;
+              res_ns[t] = 0;
+              res_st[t] = (int)(S.status | 1u | 64u);
+              res_pend[t] = 0;
+              code = (code & ~256) | 512;   // done: phase 2 skips it
+            }
+          }
+        }
+        prm[7 * kS1Group + t] = double(code);
       }
     }
     __syncthreads();
@@ -113,6 +128,16 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
       if (g * Q * G + i >= n) break;              // CTA-uniform: no team has a source i
       const int code = (i < cnt) ? (int)prm[7 * kS1Group + i] : 0;
       const bool active = (code & 256) != 0;            // team-uniform
+      if (Q == 1 && !active) {                          // nothing to do for this source (CTA-uniform with one team)
+        if (t == 0 && i < cnt && !(code & 512)) {       // invalid parameters: NaN out, status 8
+          res_mu[i] = nan("");
+          res_err[i] = nan("");
+          res_ns[i] = 0;
+          res_st[i] = 8;
+          res_pend[i] = 0;
+        }
+        continue;
+      }
       double rho = 1.0;
       int flags = 0;
       if (active) {
@@ -212,12 +237,15 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
         }
       }
       if (t == 0 && i < cnt) {
-        if (!active) {   // invalid parameters: NaN out, status 8
+        if (!active) {   // invalid parameters: NaN out, status 8 (done by the point-source tests: nothing to write)
+          if (code & 512) {
+          } else {
           res_mu[i] = nan("");
           res_err[i] = nan("");
           res_ns[i] = 0;
           res_st[i] = 8;
           res_pend[i] = 0;
+          }
         } else {
           uint32_t status = (uint32_t)(code & 255);
           if (!finite) status |= 16u;

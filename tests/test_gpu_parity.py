@@ -173,6 +173,59 @@ def test_adaptive_paper_workloads(ctx, name, kw):
     assert (st & 1).mean() > 0.999
 
 
+@pytest.fixture(scope="module")
+def ctx_ps():
+    import paper_2501_03322_b200 as P
+    c = P.Context(1 << 22, point_source_test=1)
+    yield c
+    c.close()
+
+
+@pytest.mark.parametrize("name,kw", [("config3", {}), ("config4", {}), ("config5", {}), ("config2", {}),
+                                     ("fig5_map", dict(case="resonant")), ("fig7_grid", {}), ("lowq_sweep", {})])
+def test_point_source_tests_against_oracle(ctx_ps, name, kw):
+    """with point_source_test = 1 the sources that pass the quadrupole and ghost-image tests
+    get the point-source magnification plus its quadrupole term.  Decisions and values against the oracle's twin;
+    the whole result (accepted or contour) against the converged reference at the acceptance bar."""
+    import paper_2501_03322_b200 as P
+    wl = _subsample(W.get(name, **kw), 3000, 31)
+    for tol in (1e-4, 1e-6):
+        g = ctx_ps.magnify_workload(wl, tol)
+        o = api.point_source(wl, tol, prec=0)
+        acc = (g["status"].astype(np.uint32) & P.TWK_ST_POINT) != 0
+        assert (acc == o["accept"]).mean() > 0.995                   # a borderline ratio may flip
+        both = acc & o["accept"]
+        if both.any():
+            assert np.abs(g["mu"][both] / o["mu"][both] - 1).max() < 1e-11
+            assert np.all(g["nsamples"][both] == 0) and np.allclose(g["err"][both], o["qrel"][both], rtol=1e-8)
+        assert np.all(g["nsamples"][~acc] >= 64)
+    g = ctx_ps.magnify_workload(wl, 1e-6)
+    ref = api.magnify(wl, 1e-6, mode=1, prec=0)
+    assert np.abs(g["mu"] / ref["mu"] - 1).max() <= MU_TOL
+
+
+def test_point_source_tests_full_size_against_contour(ctx_ps):
+    """Every source of every workload: where the tests accept at tol 1e-4, the value is within 1e-4 of the contour
+    path's own answer at 1e-6 (which the other tests tie to the oracle)."""
+    import paper_2501_03322_b200 as P
+    c = P.Context(1 << 22)
+    worst = 0.0
+    for wl in (W.config3(), W.config4(), W.config5(), W.fig5_map("close"), W.fig5_map("resonant"), W.fig5_map("wide"),
+               W.fig7_grid(), W.lowq_sweep(), W.config2()):
+        a = ctx_ps.magnify_workload(wl, 1e-4)
+        b = c.magnify_workload(wl, 1e-6)
+        acc = (a["status"].astype(np.uint32) & P.TWK_ST_POINT) != 0
+        d = np.abs(a["mu"] / b["mu"] - 1)
+        assert np.all(np.isfinite(a["mu"]))
+        if acc.any():
+            worst = max(worst, d[acc].max())
+            assert d[acc].max() <= 1e-4, (wl.name, d[acc].max(), int(np.argmax(np.where(acc, d, 0))))
+        same = c.magnify_workload(wl, 1e-4)                     # the other sources took the contour path unchanged
+        assert np.array_equal(a["mu"][~acc], same["mu"][~acc]) and np.array_equal(a["nsamples"][~acc], same["nsamples"][~acc])
+    c.close()
+    print("worst accepted deviation", worst)
+
+
 def test_handover_and_recompute_paths_agree():
     """Stage 1 hands the first iteration of an unfinished source to stage 2 through the hand-over arena; without a
     free slot stage 2 recomputes it.  Same arithmetic either way (up to the compiler's contraction choices in the
