@@ -297,8 +297,8 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         if (rep) status |= 4u;
         if (nonf) status |= 16u;
         if (slope_seen || slp) status |= 32u;
-        p.out_mu[src] = A / (kPi * S.rho * S.rho);
-        if (p.out_err) p.out_err[src] = E / fabs(A);
+        p.out_mu[src] = A * rcp(kPi * S.rho * S.rho);
+        if (p.out_err) p.out_err[src] = E * rcp(fabs(A));
         if (p.out_nsamples) p.out_nsamples[src] = n;
         if (p.out_status) p.out_status[src] = status;
       }

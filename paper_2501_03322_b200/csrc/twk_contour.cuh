@@ -2,6 +2,8 @@
 // See twk_device.cuh for the citation key.
 #pragma once
 
+#include <string.h>
+
 #include "twk_device.cuh"
 
 namespace twk {
@@ -14,12 +16,32 @@ namespace twk {
 //   [10..14] Re z'    z' = dz/dtheta, Eq.(10) (conj on f' restored)
 //   [15..19] Im z'
 //   [20..24] z'^z''   Eq.(10) (division by J restored)
-//   [25]    nreal (3 or 5) + 8 * point flags (kPointRepaired | kPointNonFinite | kPointSlope), stored as a double
+//   [25]    nreal (3 or 5) + 8 * point flags (kPointRepaired | kPointNonFinite | kPointSlope), an integer kept as raw bits
 // In shared memory the record is a column of a [26][TILE] array (stride = TILE, conflict-free); in the global
 // arena it is 26 contiguous doubles (stride = 1, 208 B).
 // ------------------------------------------------------------------------------------------------------------
 constexpr int kRecDoubles = 26;
 constexpr int kZX = 0, kZY = 5, kPX = 10, kPY = 15, kW = 20, kNR = 25;
+
+TWK_HD int code_of(double d) {
+#ifdef __CUDA_ARCH__
+  return (int)__double_as_longlong(d);
+#else
+  long long v;
+  memcpy(&v, &d, 8);
+  return (int)v;
+#endif
+}
+TWK_HD double code_as_double(int c) {
+#ifdef __CUDA_ARCH__
+  return __longlong_as_double((long long)c);
+#else
+  long long v = c;
+  double d;
+  memcpy(&d, &v, 8);
+  return d;
+#endif
+}
 
 struct RecRef {
   double* base;
@@ -28,8 +50,11 @@ struct RecRef {
   TWK_HD cd z(int slot) const { return mk(base[(kZX + slot) * stride], base[(kZY + slot) * stride]); }
   TWK_HD cd zp(int slot) const { return mk(base[(kPX + slot) * stride], base[(kPY + slot) * stride]); }
   TWK_HD double w(int slot) const { return base[(kW + slot) * stride]; }
-  TWK_HD int nreal() const { return int(base[kNR * stride]) & 7; }
-  TWK_HD int point_flags() const { return int(base[kNR * stride]) >> 3; }
+  // element kNR holds an integer code as raw bits (no int <-> double conversion on the hot path)
+  TWK_HD int code() const { return code_of(base[kNR * stride]); }
+  TWK_HD int nreal() const { return code() & 7; }
+  TWK_HD int point_flags() const { return code() >> 3; }
+  TWK_HD void set_code(int c) const { base[kNR * stride] = code_as_double(c); }
 };
 
 constexpr int kPointRepaired = 1;   // parity sum was not -1 and was repaired (G-5)
@@ -62,7 +87,7 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
       // A delta + B conj(delta)
       eta[k] = mk(ex + fma(ax + bx, dx, (by - ay) * dy), ey + fma(ay + by, dx, (ax - bx) * dy));
     }
-    solved = quintic_roots_seeded(c, eta);
+    solved = quintic_roots_seeded(c, eta, seeds[30 * seed_stride] != 0.0);
   }
   if (!solved) {
     TWK_COUNT(cold_solve);
@@ -164,7 +189,7 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     rec.at(kZX + 4) = eB.x + L.z2;
     rec.at(kZY + 4) = eB.y;
   }
-  rec.at(kNR) = double(nreal + 8 * flags);
+  rec.set_code(nreal + 8 * flags);
   if (out_count) *out_count = (int8_t)nreal;
   return flags;
 }
@@ -181,16 +206,19 @@ TWK_HD int point_solve(const Lens& L, cd zc, double rho, double theta, RecRef re
 //   [10..14] Re A_k, [15..19] Im A_k, [20..24] Re B_k, [25..29] Im B_k
 //                                      first-order response of root k to a displacement delta of the source:
 //                                      d eta_k = A_k delta + B_k conj(delta)
+//   [30]                               1 when two roots are closer than 1e-6 of the roots' scale (next to a planet of
+//                                      tiny q): the seeded solve then also verifies the PRODUCT of the roots
 // The quintic's roots are the fixed points (real images) and the 2-cycle (ghost pair) of T(z) = zeta - conj f(z)
 // (G-1): z_a = zeta - conj f(z_b), z_b = zeta - conj f(z_a), with z_b = z_a for a real image.
 // Differentiating both and eliminating dz_b gives dz_a (1 - f'(w_a) f'(z_a)) = delta - f'(w_a) conj(delta) with
 // w_a = conj(z_b) = conj(zeta) - f(z_a); conj(f'(z_b)) = f'(conj z_b) because both lenses are on the real axis.  For
 // a real image this is Eq.(10)'s z'.  A prediction is kept only when the shift rho (|A| + |B|) stays below
 // a quarter of the distance to the nearest other root (next to a caustic 1/J blows up); otherwise A = B = 0.
-constexpr int kSeedDoubles = 30;
+constexpr int kSeedDoubles = 31;
 
 TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int stride) {
   cd c[6], eta[5];
+  double dmin2_all = 1e300;
   const cd y = mk(zc.x - L.z2, zc.y);
   coeffs_eq6(y, L.s, L.m2, c);
   {
@@ -223,6 +251,7 @@ TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int st
       A = mk(0.0, 0.0);
       B = mk(0.0, 0.0);
     }
+    dmin2_all = fmin(dmin2_all, dmin2);
     seeds[k * stride] = eta[k].x;
     seeds[(5 + k) * stride] = eta[k].y;
     seeds[(10 + k) * stride] = A.x;
@@ -230,6 +259,8 @@ TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int st
     seeds[(20 + k) * stride] = B.x;
     seeds[(25 + k) * stride] = B.y;
   }
+  const double scale = abs1(eta[0]) + abs1(eta[1]) + abs1(eta[2]) + abs1(eta[3]) + abs1(eta[4]);
+  seeds[30 * stride] = (dmin2_all < 1e-12 * scale * scale) ? 1.0 : 0.0;
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -533,7 +564,7 @@ TWK_HD void demote_pair(const RecRef& S, int kp, int km) {
   S.at(kZY + 1) = gp.y;
   S.at(kZX + 4) = gm.x;
   S.at(kZY + 4) = gm.y;
-  S.at(kNR) = double(3 + 8 * (S.point_flags() | kPointSlope));
+  S.set_code(3 + 8 * (S.point_flags() | kPointSlope));
 }
 
 }  // namespace twk

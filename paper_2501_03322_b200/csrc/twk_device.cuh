@@ -353,7 +353,7 @@ TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev) {
   return conv;
 }
 
-TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5]) {
+TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product) {
   double prev[5];
 #pragma unroll
   for (int k = 0; k < 5; ++k) prev[k] = 0.0;
@@ -372,13 +372,17 @@ TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5]) {
   for (int it = 2; it < 22; ++it) {
     if (done == 31u || (it >= 10 && !recovered)) {
       if (done == 31u) {
-        // verification by Vieta: the sum of the roots (absolute, on the scale of the largest) and their product
-        // (relative: two chains on one of two tiny neighbouring roots next to a q = 1e-9 planet change the sum by
-        // 1e-9 of its scale but the product by their relative distance)
+        // verification by Vieta: the sum of the roots (absolute, on the scale of the largest) and, for sources
+        // flagged by centre_seeds (two roots closer than 1e-6 of the scale: next to a q = 1e-9 planet two chains on
+        // one of two tiny neighbouring roots change the sum by 1e-9 of its scale, below this test), their product
+        // (relative)
         const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
-        const cd prod = ((r[0] * r[1]) * (r[2] * r[3])) * r[4];
-        const cd dp = prod * c[5] + c[0];                 // prod = -c0/c5
-        if (abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale && abs1(dp) <= 1e-9 * abs1(c[0])) return true;
+        bool ok = abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale;
+        if (check_product) {
+          const cd prod = ((r[0] * r[1]) * (r[2] * r[3])) * r[4];
+          ok = ok && abs1(prod * c[5] + c[0]) <= 1e-9 * abs1(c[0]);          // prod = -c0/c5
+        }
+        if (ok) return true;
       }
       if (recovered) break;
       recovered = true;

@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
             }
           }
         }
-        prm[7 * kS1Group + t] = double(code);
+        prm[7 * kS1Group + t] = code_as_double(code);
       }
     }
     __syncthreads();
@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
     const int cnt = (int)((n - base < G) ? (n > base ? n - base : 0) : G);   // of this team
     for (int i = 0; i < G; ++i) {
       if (g * Q * G + i >= n) break;              // CTA-uniform: no team has a source i
-      const int code = (i < cnt) ? (int)prm[7 * kS1Group + i] : 0;
+      const int code = (i < cnt) ? code_of(prm[7 * kS1Group + i]) : 0;
       const bool active = (code & 256) != 0;            // team-uniform
       if (Q == 1 && !active) {                          // nothing to do for this source (CTA-uniform with one team)
         if (t == 0 && i < cnt && !(code & 512)) {       // invalid parameters: NaN out, status 8
@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
 #pragma unroll
       for (int qq = 0; qq < Q; ++qq) {
         const double Aq = sc[qq * 4] + sc[qq * 4 + 2], Eq = sc[qq * 4 + 1] + sc[qq * 4 + 3];
-        const bool act = ((g * Q + qq) * G + i < n) && (((int)prm_all[(qq * kS1ParamRows + 7) * kS1Group + i]) & 256);
+        const bool act = ((g * Q + qq) * G + i < n) && (code_of(prm_all[(qq * kS1ParamRows + 7) * kS1Group + i]) & 256);
         const bool fin = isfinite(Aq) && isfinite(Eq);
         const bool pd = act && fin && !(Eq <= p.tol * fabs(Aq)) && !p.final_stage;   // stop rule P:272
         any_pend = any_pend || pd;
@@ -254,8 +254,8 @@ __global__ void __launch_bounds__(Q * kThreads, kMinBlocks) stage1_kernel(Stage1
           if (flags & kPointRepaired) status |= 4u;
           if (flags & kPointNonFinite) status |= 16u;
           if (flags & kPointSlope) status |= 32u;
-          res_mu[i] = A / (kPi * rho * rho);
-          res_err[i] = E / fabs(A);
+          res_mu[i] = A * rcp(kPi * rho * rho);
+          res_err[i] = E * rcp(fabs(A));
           res_ns[i] = kThreads;
           res_st[i] = (int)status;
           res_pend[i] = pend ? 1 : 0;
