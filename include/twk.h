@@ -16,6 +16,8 @@
  *    frees, reallocates or retains them.  "HOST" pointers are ordinary host memory.
  *  - complex arrays are interleaved (re, im) doubles.
  *  - Device-pointer calls are asynchronous on `stream` and perform no host synchronisation.
+ *  - A context owns ONE workspace: its calls must be issued on one stream at a time (stream order serialises them);
+ *    use one context per stream for concurrent batches.  One context per device; create it with that device current.
  *  - Return value: TWK_OK or a negative TWK_E* code from synchronous argument validation / CUDA runtime errors.
  *    Device-side problems never abort a call: they set per-source status bits (TWK_ST_*).
  *  - There is no CPU fallback: every entry point that computes needs a CUDA device.
@@ -70,6 +72,8 @@ typedef struct {
                         /* (formulas derived in DESIGN.md, readings N1-a..c).  Sources that pass get that value  */
                         /* (status TWK_ST_POINT, out_err = relative size of the quadrupole term, out_nsamples = 0) and  */
                         /* skip the contour.  Default 0: every source takes the contour path.                           */
+  int frame;            /* frame of the zeta passed in: 0 = centre of mass (the paper's, Eq.(2)); 1 = primary lens at   */
+                        /* the origin (z1 = -q s/(1+q) is added to every zeta; BASELINE configs 1 and 2 are stated so)  */
 } twk_options;
 
 /* Fill *opt with the defaults above. */

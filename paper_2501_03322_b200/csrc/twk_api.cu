@@ -67,7 +67,7 @@ Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
 bool valid_options(const twk_options& o) {
   return o.samples_per_iter == twk::kThreads && o.initial_samples == twk::kThreads && o.max_samples >= twk::kThreads &&
          o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1) && o.handoff_slots >= -1 && o.slope_gate >= 0.0 && o.slope_cos >= 0.0 && o.slope_cos <= 1.0 &&
-         (o.point_source_test == 0 || o.point_source_test == 1);
+         (o.point_source_test == 0 || o.point_source_test == 1) && (o.frame == 0 || o.frame == 1);
 }
 
 int cuda_fail(cudaError_t e) {
@@ -85,12 +85,8 @@ int cuda_fail(cudaError_t e) {
 // stage 1 with Q teams of 64 threads per CTA; resident CTAs per SM chosen so that 12 warps are resident
 template <int Q, int kMinBlocks>
 void launch_stage1_q(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t stream) {
-  const size_t smem = twk::stage1_smem_bytes<Q>();
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(twk::stage1_kernel<Q, kMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
-  }
+  const size_t smem = twk::stage1_smem_bytes<Q>();   // below the 48 KB default limit: no opt-in needed
+  static_assert(twk::stage1_smem_bytes<Q>() <= 48 * 1024, "stage-1 shared memory needs the opt-in attribute");
   // groups of up to 64 sources per CTA pass; a small batch takes smaller groups so that every resident CTA gets work
   const long long resident = (long long)sms * kMinBlocks;
   long long group = (n_sources + resident * Q - 1) / (resident * Q);
@@ -137,6 +133,7 @@ void twk_default_options(twk_options* opt) {
   opt->slope_gate = 1e-5;
   opt->slope_cos = 0.70710678118654752;
   opt->point_source_test = 0;
+  opt->frame = 0;
 }
 
 size_t twk_workspace_bytes(const twk_options* opt, size_t max_sources) {
@@ -224,7 +221,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
   // counters: [0] cursor1, [1] count1 (stage-2 worklist), [2] cursor2, [3] count2 (stage-3 worklist), [4] cursor3
   TWK_CUDA(cudaMemsetAsync(counters, 0, 64, stream));
   twk::AdaptArgs a{};
-  a.b = twk::Batch{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources};
+  a.b = twk::Batch{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame};
   a.tol = rel_tol;
   a.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
   a.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
@@ -305,7 +302,7 @@ int twk_images_fixed(twk_ctx* ctx, size_t n_models, const double* s, const doubl
   if (n_sources == 0) return TWK_OK;
   if (N < 4) return TWK_EINVAL;
   cudaStream_t stream = (cudaStream_t)stream_;
-  twk::Batch b{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources};
+  twk::Batch b{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame};
   const size_t smem = (size_t)(twk::kRecDoubles * kFixedTile + 2 * twk::kRecDoubles + 2 * (kFixedTile / 32)) * 8;
   const long long resident = (long long)ctx->sms * 8;
   const int grid = (int)((long long)n_sources < resident ? (long long)n_sources : resident);

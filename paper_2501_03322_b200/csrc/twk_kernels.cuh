@@ -31,6 +31,7 @@ struct Batch {
   const int32_t* model_id;   // may be null
   const double* zeta;        // [n][2]
   long long n_models, n_sources;
+  int frame;                 // 0: zeta in the centre-of-mass frame (Eq.2); 1: primary at the origin (zeta + z1 is used)
 };
 
 struct SourceParams {
@@ -51,6 +52,7 @@ __device__ __forceinline__ SourceParams load_source(const Batch& b, long long sr
             isfinite(P.zc.y) && m >= 0 && m < b.n_models;
   P.status = (P.valid && s >= 0.1 && s <= 10.0 && q >= 1e-9) ? 0u : 8u;
   P.L = make_lens(P.valid ? s : 1.0, P.valid ? q : 1.0);
+  if (b.frame == 1) P.zc.x += P.L.z2 - P.L.s;   // z1 = -q s / (1 + q) = z2 - s  (reading F-1)
   return P;
 }
 

@@ -286,6 +286,21 @@ def test_slope_detector_like_for_like(slope_cos):
         assert fired > 20          # nothing is perpendicular enough: every crossing piece is deleted
 
 
+def test_frame_option(ctx):
+    """frame = 1: the caller's zeta has the primary at the origin (BASELINE configs 1, 2); the library adds z1."""
+    import paper_2501_03322_b200 as P
+    wl = W.config2().subset(np.arange(4500, 5500))
+    q, s = wl.q[0], wl.s[0]
+    z1 = -q * s / (1 + q)
+    shifted = W.Workload("c2p", wl.s, wl.q, wl.rho, wl.model_id, wl.zeta - np.array([z1, 0.0]), wl.rel_tol)
+    c = P.Context(2048, frame=1)
+    a = c.magnify_workload(shifted, 1e-4)
+    b = ctx.magnify_workload(wl, 1e-4)
+    c.close()
+    d = np.abs(a["mu"] / b["mu"] - 1)        # zeta differs by a rounding of the shift; the sampler amplifies it
+    assert np.median(d) < 1e-12 and d.max() < 1e-5 and (a["nsamples"] == b["nsamples"]).mean() > 0.99
+
+
 def test_edge_cases(ctx):
     import torch
     import paper_2501_03322_b200 as P
