@@ -208,6 +208,9 @@ static int check_batch(twk_ctx* ctx, size_t n_models, const double* s, const dou
   return TWK_OK;
 }
 
+static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, double* out_mu, double* out_err,
+                        int32_t* out_nsamples, uint32_t* out_status, void* stream_);
+
 int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho, size_t n_sources,
                 const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu, double* out_err,
                 int32_t* out_nsamples, uint32_t* out_status, void* stream_) {
@@ -215,13 +218,34 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
   if (rc != TWK_OK) return rc;
   if (n_sources == 0) return TWK_OK;
   if (!out_mu || !(rel_tol > 0.0)) return TWK_EINVAL;
+  const twk::Batch b{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame,
+                     nullptr, nullptr, nullptr, nullptr, nullptr};
+  return magnify_impl(ctx, b, rel_tol, out_mu, out_err, out_nsamples, out_status, stream_);
+}
+
+int twk_magnify_lightcurve(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                           const double* t0, const double* u0, const double* tE, const double* alpha, size_t n_sources,
+                           const int32_t* model_id, const double* t, double rel_tol, double* out_mu, double* out_err,
+                           int32_t* out_nsamples, uint32_t* out_status, void* stream_) {
+  const int rc = check_batch(ctx, n_models, s, q, rho, n_sources, model_id, t);
+  if (rc != TWK_OK) return rc;
+  if (n_sources == 0) return TWK_OK;
+  if (!t0 || !u0 || !tE || !alpha || !out_mu || !(rel_tol > 0.0)) return TWK_EINVAL;
+  const twk::Batch b{s, q, rho, model_id, nullptr, (long long)n_models, (long long)n_sources, ctx->opt.frame,
+                     t, t0, u0, tE, alpha};
+  return magnify_impl(ctx, b, rel_tol, out_mu, out_err, out_nsamples, out_status, stream_);
+}
+
+static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, double* out_mu, double* out_err,
+                        int32_t* out_nsamples, uint32_t* out_status, void* stream_) {
+  const size_t n_sources = (size_t)batch.n_sources;
   cudaStream_t stream = (cudaStream_t)stream_;
   const Plan& P = ctx->plan;
   int* counters = reinterpret_cast<int*>(ctx->ws + ctx->lay.counters);
   // counters: [0] cursor1, [1] count1 (stage-2 worklist), [2] cursor2, [3] count2 (stage-3 worklist), [4] cursor3
   TWK_CUDA(cudaMemsetAsync(counters, 0, 64, stream));
   twk::AdaptArgs a{};
-  a.b = twk::Batch{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame};
+  a.b = batch;
   a.tol = rel_tol;
   a.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
   a.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
@@ -302,7 +326,8 @@ int twk_images_fixed(twk_ctx* ctx, size_t n_models, const double* s, const doubl
   if (n_sources == 0) return TWK_OK;
   if (N < 4) return TWK_EINVAL;
   cudaStream_t stream = (cudaStream_t)stream_;
-  twk::Batch b{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame};
+  twk::Batch b{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame,
+               nullptr, nullptr, nullptr, nullptr, nullptr};
   const size_t smem = (size_t)(twk::kRecDoubles * kFixedTile + 2 * twk::kRecDoubles + 2 * (kFixedTile / 32)) * 8;
   const long long resident = (long long)ctx->sms * 8;
   const int grid = (int)((long long)n_sources < resident ? (long long)n_sources : resident);

@@ -32,6 +32,13 @@ struct Batch {
   const double* zeta;        // [n][2]
   long long n_models, n_sources;
   int frame;                 // 0: zeta in the centre-of-mass frame (Eq.2); 1: primary at the origin (zeta + z1 is used)
+  // light-curve front end (twk_magnify_lightcurve): when `t` is set, zeta = -(tau + i u0) e^{i alpha},
+  // tau = (t - t0) / tE, is computed here from the epoch and the model's trajectory parameters; `zeta` is unused
+  const double* t;           // [n_sources] epochs, or null
+  const double* t0;          // [n_models]
+  const double* u0;          // [n_models]
+  const double* tE;          // [n_models]
+  const double* alpha;       // [n_models]
 };
 
 struct SourceParams {
@@ -44,12 +51,20 @@ struct SourceParams {
 
 __device__ __forceinline__ SourceParams load_source(const Batch& b, long long src) {
   SourceParams P;
-  const long long m = b.model_id ? (long long)b.model_id[src] : (b.n_models == 1 ? 0 : src);
+  const long long m_in = b.model_id ? (long long)b.model_id[src] : (b.n_models == 1 ? 0 : src);
+  const long long m = (m_in >= 0 && m_in < b.n_models) ? m_in : 0;   // never read outside the model arrays
   const double s = b.s[m], q = b.q[m], rho = b.rho[m];
-  P.zc = mk(b.zeta[2 * src], b.zeta[2 * src + 1]);
+  if (b.t) {
+    const double tau = (b.t[src] - b.t0[m]) / b.tE[m], u0 = b.u0[m];
+    double sa, ca;
+    sincos(b.alpha[m], &sa, &ca);
+    P.zc = mk(-(tau * ca - u0 * sa), -(tau * sa + u0 * ca));
+  } else {
+    P.zc = mk(b.zeta[2 * src], b.zeta[2 * src + 1]);
+  }
   P.rho = rho;
   P.valid = (s > 0.0) && (q > 0.0) && (rho > 0.0) && isfinite(s) && isfinite(q) && isfinite(rho) && isfinite(P.zc.x) &&
-            isfinite(P.zc.y) && m >= 0 && m < b.n_models;
+            isfinite(P.zc.y) && m_in >= 0 && m_in < b.n_models;
   P.status = (P.valid && s >= 0.1 && s <= 10.0 && q >= 1e-9) ? 0u : 8u;
   P.L = make_lens(P.valid ? s : 1.0, P.valid ? q : 1.0);
   if (b.frame == 1) P.zc.x += P.L.z2 - P.L.s;   // z1 = -q s / (1 + q) = z2 - s  (reading F-1)

@@ -286,6 +286,37 @@ def test_slope_detector_like_for_like(slope_cos):
         assert fired > 20          # nothing is perpendicular enough: every crossing piece is deleted
 
 
+def test_lightcurve_front_end(ctx):
+    """twk_magnify_lightcurve computes zeta(t) = -(tau + i u0) e^{i alpha} on the device; same
+    magnifications as twk_magnify fed with the generator's zeta (workloads.trajectory)."""
+    import torch
+    import paper_2501_03322_b200 as P
+    rng = np.random.default_rng(77)
+    n_models, n_ep = 48, 120
+    s = np.exp(rng.uniform(np.log(0.3), np.log(3.0), n_models))
+    q = np.exp(rng.uniform(np.log(1e-5), 0.0, n_models))
+    rho = np.exp(rng.uniform(np.log(1e-4), np.log(1e-2), n_models))
+    u0 = rng.uniform(-0.1, 0.1, n_models)
+    alpha = rng.uniform(0.0, 2 * np.pi, n_models)
+    t0 = rng.uniform(-5.0, 5.0, n_models)
+    tE = rng.uniform(10.0, 40.0, n_models)
+    t = (t0[:, None] + tE[:, None] * np.linspace(-1.5, 1.5, n_ep)[None, :]).ravel()
+    mid = np.repeat(np.arange(n_models, dtype=np.int32), n_ep)
+    tau = (t - t0[mid]) / tE[mid]
+    zc = W.trajectory(tau, u0[mid], alpha[mid])
+    wl = W.Workload("lc", s, q, rho, mid, np.ascontiguousarray(np.stack([zc.real, zc.imag], 1)), 1e-4)
+    ref = ctx.magnify_workload(wl, 1e-4)
+    f = lambda a, dt=torch.float64: torch.from_numpy(np.ascontiguousarray(a)).to("cuda", dt)
+    r = ctx.twk_magnify_lightcurve(f(s), f(q), f(rho), f(t0), f(u0), f(tE), f(alpha), f(t), f(mid, torch.int32), 1e-4)
+    mu = r["mu"].cpu().numpy()
+    d = np.abs(mu / ref["mu"] - 1)
+    assert np.median(d) < 1e-12 and d.max() < 1e-5
+    assert (r["nsamples"].cpu().numpy() == ref["nsamples"]).mean() > 0.99
+    o = api.magnify(wl, 1e-6, mode=1)
+    r6 = ctx.twk_magnify_lightcurve(f(s), f(q), f(rho), f(t0), f(u0), f(tE), f(alpha), f(t), f(mid, torch.int32), 1e-6)
+    assert np.abs(r6["mu"].cpu().numpy() / o["mu"] - 1).max() <= MU_TOL
+
+
 def test_frame_option(ctx):
     """frame = 1: the caller's zeta has the primary at the origin (BASELINE configs 1, 2); the library adds z1."""
     import paper_2501_03322_b200 as P
