@@ -82,30 +82,23 @@ int cuda_fail(cudaError_t e) {
 
 }  // namespace
 
-// stage 1 with Q teams of 64 threads per CTA; resident CTAs per SM chosen so that 12 warps are resident
-template <int Q, int kMinBlocks>
-void launch_stage1_q(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t stream) {
-  const size_t smem = twk::stage1_smem_bytes<Q>();   // below the 48 KB default limit: no opt-in needed
-  static_assert(twk::stage1_smem_bytes<Q>() <= 48 * 1024, "stage-1 shared memory needs the opt-in attribute");
+// stage 1: persistent CTAs of 64 threads, kS1CtasPerSM per SM.  Measured on config 3 (B200) with several 64-thread
+// teams per CTA kept in step by CTA-wide barriers: 1 x 6 CTAs/SM 36.5 ms, 2 x 3: 36.0, 3 x 2: 38.3, 4 x 1: 47.8,
+// 6 x 1: 43.7 -- coupling the teams costs more than the shared instruction stream saves, so one team per CTA it is.
+void launch_stage1(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t stream) {
+  const size_t smem = twk::stage1_smem_bytes();   // below the 48 KB default limit: no opt-in needed
+  static_assert(twk::stage1_smem_bytes() <= 48 * 1024, "stage-1 shared memory needs the opt-in attribute");
   // groups of up to 64 sources per CTA pass; a small batch takes smaller groups so that every resident CTA gets work
-  const long long resident = (long long)sms * kMinBlocks;
-  long long group = (n_sources + resident * Q - 1) / (resident * Q);
+  const long long resident = (long long)sms * twk::kS1CtasPerSM;
+  long long group = (n_sources + resident - 1) / resident;
   group = group < 4 ? 4 : (group > twk::kS1Group ? twk::kS1Group : group);
   a.group = (int)group;
-  const long long groups = (n_sources + Q * group - 1) / (Q * group);
+  const long long groups = (n_sources + group - 1) / group;
   const int grid = (int)(groups < resident ? groups : resident);
-  twk::stage1_kernel<Q, kMinBlocks><<<grid, Q * twk::kThreads, smem, stream>>>(a);
-}
-
-void launch_stage1(int teams, int sms, long long groups /* n_sources */, const twk::Stage1Args& a, cudaStream_t stream) {
-  // measured on config 3 (B200): 1 team x 6 CTAs/SM 36.5 ms, 2 x 3: 36.0, 3 x 2: 38.3, 4 x 1: 47.8, 6 x 1: 43.7 --
-  // coupling the teams through CTA-wide barriers costs more than the shared instruction stream saves
-  (void)teams;
-  launch_stage1_q<1, 6>(sms, groups, a, stream);
+  twk::stage1_kernel<<<grid, twk::kThreads, smem, stream>>>(a);
 }
 
 struct twk_ctx {
-  int stage1_teams;
   twk_options opt;
   size_t max_sources;
   int sms;
@@ -167,7 +160,6 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   c->last_launches = 0;
   c->timing = 0;
   c->ev_used = 0;
-  c->stage1_teams = 1;
   for (int i = 0; i < 5; ++i) c->ev[i] = nullptr;
   cudaError_t e = cudaMalloc((void**)&c->ws, c->lay.total);
   if (e != cudaSuccess) {
@@ -282,7 +274,7 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a1.out_err = out_err;
     a1.out_nsamples = out_nsamples;
     a1.out_status = out_status;
-    launch_stage1(ctx->stage1_teams, ctx->sms, (long long)n_sources, a1, stream);
+    launch_stage1(ctx->sms, (long long)n_sources, a1, stream);
     ++launches;
     mark();
   }
