@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl twk|reference] [--workload config3]
 
-A "step" is one pass of the whole hot path (stage 1 -> compaction -> stage 2 -> stage 3, all SURVEY 8(a) rows) over
+A "step" is one pass of the whole hot path (stage 1 -> stage 2 -> stage 3 of twk_magnify, all SURVEY 8(a) rows) over
 one batch of synthetic input: config 3 = 4,096 seeded lens models x 1,000 epochs = 4,096,000 source positions at
 relative tolerance 1e-4.  `value` = magnifications/s with inputs resident in HBM; `e2e` = the same through
 twk_magnify_host with pinned HOST buffers (H2D + D2H inside the timed region).  Rank 0 prints ONE JSON line.
