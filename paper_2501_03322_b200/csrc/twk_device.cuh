@@ -2,9 +2,10 @@
 //
 //   a1  boundary sample            zeta_j = zeta_c + rho e^{i theta_j}, zeta'_j = i rho e^{i theta_j}
 //   a2  coefficient builder        Eq.(6), planet frame
-//   a3  quintic solve              Laguerre + forward deflation + Newton polish on the full polynomial
+//   a3  quintic solve              seeded Newton on the full polynomial (Vieta-verified, Vieta recovery); cold solver:
+//                                  Laguerre + forward deflation + Newton polish
 //   a4  per-root lens quantities   f', f'', R (Eq.12), J (Eq.7), z' and z'^z'' (Eq.10, repaired)
-//   a5  ghost filter               residual detector, 2-cycle reading
+//   a5  ghost filter               residual detector, 2-cycle reading; slope detector at count changes
 //   a6  contour linker             per-parity minimum-total-distance matching, creation / annihilation
 //   a7  area + error per interval  Eq.(9)-(11), Eq.(17)-(18)
 //

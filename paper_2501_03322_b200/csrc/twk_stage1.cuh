@@ -1,6 +1,6 @@
 // twk_stage1.cuh -- stage 1 of twk_magnify: the first iteration (64 uniform boundary samples) of EVERY source.
 //
-// One 64-thread CTA takes a group of 64 consecutive sources from an atomic cursor:
+// One 64-thread CTA takes a group of up to 64 consecutive sources from an atomic cursor:
 //   phase 1  thread i cold-solves the point source at the CENTRE of source i (Laguerre + deflation): its five
 //            planet-frame roots and their first-order response to a source displacement are the seeds of that
 //            source's boundary samples (centre_seeds(), twk_contour.cuh);
@@ -10,7 +10,9 @@
 //            the refinement worklist (a9) and its whole first-iteration state -- 64 records, 64 interval
 //            pieces, seeds -- is handed to stage 2 through the hand-over arena (coalesced 512 B rows);
 //   phase 3  coalesced write of the group's results.
-// Per-source state of a finished source never leaves the SM: records [26][64], seeds [30][64], parameters [8][64].
+// With the point-source option (N1) phase 1 also runs the quadrupole and ghost-image tests; sources that pass
+// are finished there.  Per-source state of a finished source never leaves the SM: records [26][64], seeds [31][64],
+// parameters [8][64].
 #pragma once
 
 #include "twk_kernels.cuh"
