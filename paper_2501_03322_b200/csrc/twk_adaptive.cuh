@@ -133,8 +133,12 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         const bool raw = !(W > 0.0);
         if (raw) W = E;
         const double scale = double(kThreads) / W;
-        newint[t] = -1;
+        // Each interval marks the first quantile it owns (cint: interval | one-past-last quantile << 16, cth: its
+        // exclusive cumulative weight); afterwards every quantile finds its owner by a max-scan over the marks and
+        // computes its own angle: 64 angles in parallel even when one interval owns them all.
+        cint[t] = -1;
         double carry = 0.0;
+        __syncthreads();
         for (int base = 0; base < n; base += kThreads) {
           const int i = base + t;
           const double w = (i < n) ? (raw ? er[i] : fmax(er[i] - avg, 0.0)) : 0.0;
@@ -156,18 +160,44 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
             // quantile k has target (k + 1/2)/64 * W (reading A-4); this interval owns those in [cum_excl, cum_incl)
             const int klo = min(kThreads, max(0, (int)ceil(cum_excl * scale - 0.5)));
             const int khi = min(kThreads, max(0, (int)ceil(cum_incl * scale - 0.5)));
-            const double th0 = theta[i];
-            const double hi = (i + 1 < n) ? theta[i + 1] : kTwoPi;
-            const double inv_w = rcp(w);
-            for (int k = klo; k < khi; ++k) {
-              const double target = (double(k) + 0.5) / double(kThreads) * W;
-              const double frac = (target - cum_excl) * inv_w;
-              const double th = fma(frac, hi - th0, th0);              // linear interpolation
-              newth[k] = (th > th0 && th < hi) ? th : nan("");
-              newint[k] = i;
+            if (khi > klo) {
+              cint[klo] = i | (khi << 16);
+              cth[klo] = cum_excl;
             }
           }
           carry += w0 + w1;
+        }
+        __syncthreads();
+        {
+          // owner of quantile t: the last mark at a position <= t (inclusive max-scan over the 64 positions)
+          int pos = (cint[t] >= 0) ? t : -1;
+  #pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, pos, o);
+            if (lane >= o) pos = max(pos, y);
+          }
+          if (lane == 31) iscr[1 + warp] = pos;
+          __syncthreads();
+          if (warp == 1) pos = max(pos, iscr[1]);
+          int own = -1;
+          double th = 0.0;
+          if (pos >= 0) {
+            const int mark = cint[pos];
+            const int i = mark & 0xffff, khi = mark >> 16;
+            if (t < khi) {
+              const double cum_excl = cth[pos];
+              const double w = raw ? er[i] : fmax(er[i] - avg, 0.0);
+              const double th0 = theta[i];
+              const double hi = (i + 1 < n) ? theta[i + 1] : kTwoPi;
+              const double target = (double(t) + 0.5) / double(kThreads) * W;
+              const double frac = (target - cum_excl) * rcp(w);
+              th = fma(frac, hi - th0, th0);                           // linear interpolation
+              if (!(th > th0 && th < hi)) th = nan("");
+              own = i;
+            }
+          }
+          newth[t] = th;
+          newint[t] = own;
         }
         __syncthreads();
         // ---- drop invalid / duplicate angles, compact (ballot + prefix sum) --------------------------------------
