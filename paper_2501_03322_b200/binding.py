@@ -126,7 +126,11 @@ class Context:
             lib().twk_destroy(self._h)
             self._h = C.c_void_p()
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:      # interpreter shutdown: module globals may already be gone
+            pass
 
     # -- device-pointer calls -----------------------------------------------------------------------------------
     def twk_magnify(self, s, q, rho, zeta, model_id=None, rel_tol=1e-4, out_mu=None, out_err=None, out_nsamples=None,
