@@ -91,6 +91,13 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
     int n = 0;
     hand = (p.handoff && cur < p.handoff_slots) ? p.handoff + (size_t)cur * kHandDoubles : nullptr;
     if (hand) {   // done by stage 1: take its interval pieces and seed block, use its records in place
+      // the slot was written long ago (4 GB of hand-over traffic per call has left the L2): pull its 14.6 KB back
+      // into the L2 now, the first solve hides the DRAM latency
+      {
+        const char* hb = reinterpret_cast<const char*>(hand);
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(hb + t * 128));
+        if ((t + kThreads) * 128 < kHandDoubles * 8) asm volatile("prefetch.global.L2 [%0];" ::"l"(hb + (t + kThreads) * 128));
+      }
       theta[t] = kTwoPi * double(t) / double(kThreads);
       ids[t] = (uint16_t)t;
       dA[t] = hand[kRecDoubles * kThreads + t];
