@@ -157,7 +157,8 @@ def test_full_size_config3_sampled_outputs(ctx):
 
 
 @pytest.mark.parametrize("name,kw", [("fig5_map", dict(case="close")), ("fig5_map", dict(case="resonant")),
-                                     ("fig5_map", dict(case="wide")), ("fig7_grid", {}), ("lowq_sweep", {})])
+                                     ("fig5_map", dict(case="wide")), ("fig7_grid", {}), ("lowq_sweep", {}),
+                                     ("domain_corners", {})])
 def test_adaptive_paper_workloads(ctx, name, kw):
     """the paper's own caustic-dense inputs -- the three 480 x 340 source-plane maps of Fig. 5
     (P:342), the (s, q) sweep of Fig. 7 with 30 x 30 sources per lens over the caustic, and a low-q

@@ -15,8 +15,8 @@ Conventions
   "central-caustic crossing".
 * RNG: numpy.random.default_rng(seed); arrays are drawn in the order listed, whole-array draws.
 """
-from .configs import (Workload, config1, config2, config3, config4, config5, fig1_case, fig2_case,
+from .configs import (Workload, config1, config2, config3, config4, config5, domain_corners, fig1_case, fig2_case,
                       fig5_map, fig6_case, fig7_grid, get, lowq_sweep, trajectory)
 
 __all__ = ["Workload", "config1", "config2", "config3", "config4", "config5", "fig1_case", "fig2_case",
-           "fig5_map", "fig6_case", "fig7_grid", "lowq_sweep", "get", "trajectory"]
+           "fig5_map", "fig6_case", "fig7_grid", "lowq_sweep", "domain_corners", "get", "trajectory"]

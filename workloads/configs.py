@@ -208,8 +208,21 @@ def lowq_sweep(n: int = 4000, seed: int = 250103324) -> Workload:
                     meta={"seed": seed})
 
 
+def domain_corners(n: int = 4000, seed: int = 250103325) -> Workload:
+    """The corners of the validated domain of P:374: s uniform in [0.1, 0.2] or [5, 10] (half each), q log-uniform in
+    [1e-9, 1e-7], rho log-uniform in [1e-4, 1e-2]; source centre within 3 rho of the planetary-caustic position
+    s - 1/s on the axis.  tol 1e-4."""
+    rng = np.random.default_rng(seed)
+    s = np.where(rng.random(n) < 0.5, rng.uniform(0.1, 0.2, n), rng.uniform(5.0, 10.0, n))
+    q = np.exp(rng.uniform(np.log(1e-9), np.log(1e-7), n))
+    rho = np.exp(rng.uniform(np.log(1e-4), np.log(1e-2), n))
+    zc = (s - 1.0 / s) + 3.0 * rho * (rng.uniform(-1.0, 1.0, n) + 1j * rng.uniform(-1.0, 1.0, n))
+    return Workload("domain_corners", _f64(s), _f64(q), _f64(rho), np.arange(n, dtype=np.int32), _pack(zc), 1e-4,
+                    meta={"seed": seed})
+
+
 def get(name: str, **kw) -> Workload:
     table = {"config1": config1, "config2": config2, "config3": config3, "config4": config4,
              "config5": config5, "fig1": fig1_case, "fig2": fig2_case, "fig6": fig6_case, "fig5_map": fig5_map,
-             "fig7_grid": fig7_grid, "lowq_sweep": lowq_sweep}
+             "fig7_grid": fig7_grid, "lowq_sweep": lowq_sweep, "domain_corners": domain_corners}
     return table[name](**kw)
