@@ -32,6 +32,11 @@ def lib():
         L.orc_point_source.argtypes = [C.c_int64, _D, _D, _D, C.c_int64, _I32, _D, C.c_double, C.c_int, _I8, _D, _D, _D]
         L.orc_magnify_thetas.argtypes = [C.c_double] * 6 + [C.c_int] * 5 + [_D]
         L.orc_magnify_thetas.restype = C.c_int
+        L.orc_pieces_at.argtypes = [C.c_double] * 5 + [C.c_int, _D, C.c_int, _D, _D, _I32, _I32]
+        L.orc_eval_interval_synth.argtypes = [_I32, _D, _D, _D, _I32, _D, _D, _D, C.c_double, _D]
+        L.orc_eval_interval_synth.restype = C.c_int
+        L.orc_sampler_step.argtypes = [C.c_int, _D, _D, C.c_double, C.c_int, C.c_int, _D]
+        L.orc_sampler_step.restype = C.c_int
         L.orc_rayshoot.argtypes = [C.c_double] * 9 + [C.c_int] * 4
         L.orc_rayshoot.restype = C.c_double
         _lib = L
@@ -144,3 +149,43 @@ def magnify_thetas(s, q, rho, zeta_c, rel_tol, prec=0, samples_per_iter=64, init
 def rayshoot(s, q, rho, zeta_c, box, nx, ny, sub=16, nthreads=0):
     x0, x1, y0, y1 = box
     return float(lib().orc_rayshoot(s, q, rho, complex(zeta_c).real, complex(zeta_c).imag, x0, x1, y0, y1, nx, ny, sub, nthreads))
+
+
+TERMS = ("E1", "E2", "E3", "E4", "cE1", "cE2", "cE3", "corr")
+
+
+def pieces_at(s, q, rho, zeta_c, theta, prec=0):
+    """Diagnostics: the contour over the sorted angles `theta`.  Returns dict(dA[n], err[n], terms[n,8] (see TERMS),
+    cross[n], count[n]); interval i is (theta_i, theta_{i+1}), the last one closes the loop."""
+    theta = np.ascontiguousarray(theta, dtype=np.float64)
+    n = len(theta)
+    piece, terms = np.zeros((n, 2)), np.zeros((n, 8))
+    cross, count = np.zeros(n, np.int32), np.zeros(n, np.int32)
+    lib().orc_pieces_at(s, q, rho, complex(zeta_c).real, complex(zeta_c).imag, n, _p(theta, _D), prec, _p(piece, _D),
+                        _p(terms, _D), _p(cross, _I32), _p(count, _I32))
+    return dict(dA=piece[:, 0], err=piece[:, 1], terms=terms, cross=cross, count=count)
+
+
+def eval_interval_synth(A, B, dth):
+    """Diagnostics: eval_interval on two synthetic samples.  A, B = dict(kind int[5], z complex[5], zp complex[5], w float[5]).
+    Returns dict(dA, err, terms[8], crossing)."""
+    def pack(S):
+        z = np.asarray(S["z"], dtype=np.complex128)
+        zp = np.asarray(S["zp"], dtype=np.complex128)
+        return (np.ascontiguousarray(S["kind"], dtype=np.int32), np.ascontiguousarray(np.stack([z.real, z.imag], 1).ravel()),
+                np.ascontiguousarray(np.stack([zp.real, zp.imag], 1).ravel()), np.ascontiguousarray(S["w"], dtype=np.float64))
+    ka, za, pa, wa = pack(A)
+    kb, zb, pb, wb = pack(B)
+    out = np.zeros(10)
+    c = lib().orc_eval_interval_synth(_p(ka, _I32), _p(za, _D), _p(pa, _D), _p(wa, _D), _p(kb, _I32), _p(zb, _D), _p(pb, _D),
+                                      _p(wb, _D), float(dth), _p(out, _D))
+    return dict(dA=out[0], err=out[1], terms=out[2:].copy(), crossing=int(c))
+
+
+def sampler_step(theta, err, tolA, K=64, subtract_avg_tol=1):
+    """Diagnostics: one step of the paper-style sampler on caller-given interval errors.  Returns the new angles."""
+    theta = np.ascontiguousarray(theta, dtype=np.float64)
+    err = np.ascontiguousarray(err, dtype=np.float64)
+    out = np.zeros(K)
+    m = lib().orc_sampler_step(len(theta), _p(theta, _D), _p(err, _D), float(tolA), int(K), int(subtract_avg_tol), _p(out, _D))
+    return out[:m]

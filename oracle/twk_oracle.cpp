@@ -16,7 +16,12 @@
 // (P:155-159); generalised point-source magnification sum = 1; z' and z'^z'' vs finite differences of tracked
 // images; single-lens limits (Paczynski point source, uniform-disk closed forms); large-rho limit;
 // mass-swap / reflection symmetries; brute-force ray shooting on tiny inputs; the Fig.1 / Fig.2 worked
-// examples.  Unpinned: adaptive-mode *sample positions* (only the value mu is compared).
+// examples.  tests/test_oracle_errors.py: the crossing piece Eq.(11) and the estimate Eq.(18)
+// against the closed forms of a fold model (creation and annihilation separately) and against fine integrations of
+// the same interval on real lenses; Eq.(17) term by term against 50-digit mpmath image tracks; the estimate's honesty
+// interval by interval; the sampler against hand-computed quantiles; the parity repair against Eq.(7).
+// Unpinned: adaptive-mode *sample positions* on real sources (only mu, n and status are compared); slope-detector
+// decisions at the default gate (it never fires).
 
 #include <algorithm>
 #include <cmath>
@@ -243,6 +248,10 @@ template <class R> struct Piece {
   int kp, km;    // the ghost pair of the 3-image sample next to it and must be re-judged as ghosts
   int nlinks;
   int linkL[5], linkR[5];  // root indices of the linked pairs (diagnostics / tests)
+  // diagnostics for the pins (no effect on dA / err): the interval's error estimate term by term --
+  // [0..3] Eq.(17) E1..E4 summed over the regular links, [4..6] Eq.(18) E1..E3 of the crossing, [7] the crossing's
+  // Eq.(11) correction as it entered dA (signed)
+  R terms[8];
 };
 
 template <class R>
@@ -254,6 +263,7 @@ void eval_interval(const Sample<R>& A, const Sample<R>& B, R dth, Piece<R>& P, R
   P.slope = 0;
   P.kp = P.km = -1;
   P.nlinks = 0;
+  for (int k = 0; k < 8; ++k) P.terms[k] = 0;
   int leftA[5], leftB[5], nLA = 0, nLB = 0;
   for (int par = +1; par >= -1; par -= 2) {
     int ia[5], ib[5], na = 0, nb = 0;
@@ -295,6 +305,7 @@ void eval_interval(const Sample<R>& A, const Sample<R>& B, R dth, Piece<R>& P, R
       const R E3 = R(0.1) * std::abs(dAp) * dth * dth;
       const R E4 = std::abs(p1 - p2);
       P.err += E1 + E2 + E3 + E4;
+      P.terms[0] += E1; P.terms[1] += E2; P.terms[2] += E3; P.terms[3] += E4;
     }
     for (int j = ns; j < nl; ++j) {
       if (a_small) leftB[nLB++] = lg[bestp[j]]; else leftA[nLA++] = lg[bestp[j]];
@@ -336,21 +347,26 @@ void eval_interval(const Sample<R>& A, const Sample<R>& B, R dth, Piece<R>& P, R
   const R sq = std::sqrt(std::abs(dot(S.zp[kp], S.zp[km])));
   const R dtt = std::abs(d) / sq;                                                    // Eq.(11) tilde Delta theta
   const R corr = (S.w[kp] - S.w[km]) * dtt * dtt * dtt / R(24);                      // Eq.(11)
-  R dAp, chord, E2;
-  if (creation) {   // path z- -> z+   (reading S-2)
+  // Eq.(11) enters as printed in BOTH directions (reading S-2): the + track is followed with
+  // increasing theta, the - track against it, so the pair's path is z- -> (critical curve) -> z+ at a creation and
+  // z+ -> z- at an annihilation; only the closing chord changes direction.  For the fold model
+  // z+- = zc + a d t ^ +- b sqrt(d) n ^ (d = |theta - theta_c|) the printed correction equals the area between that
+  // path and its chord exactly, with the same sign in both cases (tests/test_oracle_errors.py, fold model).
+  const R dAp = corr;
+  R chord, E2;
+  if (creation) {   // path z- -> z+
     chord = R(0.5) * wedge(zmi, d);
-    dAp = -corr;
-    E2 = R(1.5) * std::abs(dot(d, S.zp[kp] - S.zp[km]) - R(2) * std::abs(d) * sq) * dtt;   // Eq.(18), E-5
+    E2 = R(1.5) * std::abs(dot(d, S.zp[kp] - S.zp[km]) - R(2) * std::abs(d) * sq) * dtt;   // Eq.(18), E-5; '-' P:302
   } else {          // path z+ -> z-
     chord = R(0.5) * wedge(zpl, -d);
-    dAp = +corr;
-    E2 = R(1.5) * std::abs(dot(d, S.zp[kp] - S.zp[km]) + R(2) * std::abs(d) * sq) * dtt;
+    E2 = R(1.5) * std::abs(dot(d, S.zp[kp] - S.zp[km]) + R(2) * std::abs(d) * sq) * dtt;   // '+' P:302
   }
   P.crossing = creation ? +1 : -1;
   P.dA += chord + dAp;
   const R E1 = std::abs(S.w[kp] + S.w[km]) * dtt * dtt * dtt / R(48);                // Eq.(18)
   const R E3 = R(0.1) * std::abs(dAp) * dth * dth;
   P.err += E1 + E2 + E3;
+  P.terms[4] = E1; P.terms[5] = E2; P.terms[6] = E3; P.terms[7] = dAp;
 }
 
 const double kPi = 3.14159265358979323846264338327950288;
@@ -499,6 +515,62 @@ template <class R> struct Contour {
   }
 };
 
+// ---------------------------------------------------------------------------------------------------------
+// a8. One step of the paper's sampler (Fig.4): the per-interval errors are the sampling weights; the
+// normalised cumulative error is inverted at K quantiles placed uniformly on the vertical axis, with linear
+// interpolation inside the interval.  theta[] sorted, err[i] / bad[i] belong to the interval (theta_i, theta_{i+1})
+// (cyclic, the last one closes at 2 pi + theta_0); tolA = tol * |A|.
+//   A-4  quantile k sits at (k + 1/2) / K of the total weight: the only uniform placement for which K quantiles
+//        give K NEW samples (Fig.4's caption: "generates eight new samples"); k / K and (k + 1) / K each put one
+//        quantile on an existing sample.
+//   A-5  "we subtract each error by the average tolerance": w_i = max(e_i - tolA / n, 0); an interval already
+//        below its share gets no new sample.  If every weight vanishes the raw errors are used.
+//   A-7  inconsistent intervals (oracle only) share half of the quantiles.
+// Returns the new angles (those strictly inside their interval), in quantile order.
+// ---------------------------------------------------------------------------------------------------------
+template <class R>
+std::vector<R> sampler_new_thetas(const std::vector<R>& theta, const std::vector<R>& err, const std::vector<char>& bad,
+                                  R twopi, R tolA, int K, int subtract_avg_tol) {
+  const int n = (int)theta.size();
+  auto dtheta = [&](int i) { return (i + 1 < n) ? theta[i + 1] - theta[i] : twopi - theta[i] + theta[0]; };
+  int nbad = 0;
+  for (int i = 0; i < n; ++i) nbad += bad[i] ? 1 : 0;
+  std::vector<R> wgt(n);
+  const R avg = subtract_avg_tol ? tolA / R(n) : R(0);                              // P:306, A-5
+  R W = 0;
+  for (int i = 0; i < n; ++i) {
+    wgt[i] = bad[i] ? R(0) : std::max(err[i] - avg, R(0));
+    W += wgt[i];
+  }
+  if (nbad) {   // inconsistent intervals take half of the quantiles (reading A-7)
+    const R wb = (W + tolA) / R(nbad);
+    W = 0;
+    for (int i = 0; i < n; ++i) {
+      if (bad[i]) wgt[i] = wb;
+      W += wgt[i];
+    }
+  }
+  if (!(W > 0)) {
+    W = 0;
+    for (int i = 0; i < n; ++i) { wgt[i] = err[i]; W += wgt[i]; }
+  }
+  std::vector<R> cum(n + 1);
+  cum[0] = 0;
+  for (int i = 0; i < n; ++i) cum[i + 1] = cum[i] + wgt[i];
+  std::vector<R> newth;
+  for (int k = 0; k < K; ++k) {
+    const R target = (R(k) + R(0.5)) / R(K) * cum[n];                               // quantiles, A-4
+    int i = int(std::upper_bound(cum.begin(), cum.end(), target) - cum.begin()) - 1;
+    i = std::min(std::max(i, 0), n - 1);
+    while (i < n - 1 && !(wgt[i] > 0)) ++i;
+    const R frac = wgt[i] > 0 ? (target - cum[i]) / wgt[i] : R(0.5);
+    const R th = theta[i] + frac * dtheta(i);                                       // linear interpolation
+    const R hi = (i + 1 < n) ? theta[i + 1] : twopi;
+    if (th > theta[i] && th < hi) newth.push_back(th);
+  }
+  return newth;
+}
+
 template <class R>
 void magnify_one(double s, double q, double rho_, double zre, double zim, double tol, int mode, const AdaptOpt& o,
                  double* out_mu, double* out_err, int32_t* out_n, uint32_t* out_status, double* out_theta /*optional, max_samples*/) {
@@ -531,39 +603,10 @@ void magnify_one(double s, double q, double rho_, double zre, double zim, double
       if (nbad == 0 && E <= rtol * std::abs(A)) { status |= 1; break; }           // P:272, A-1
       if (n + K > o.max_samples) { status |= 2; break; }                          // P:326, A-6
       // error-weighted inverse-transform sampling
-      std::vector<R> wgt(n);
-      const R avg = o.subtract_avg_tol ? rtol * std::abs(A) / R(n) : R(0);        // P:306, A-5
-      R W = 0;
-      for (int i = 0; i < n; ++i) {
-        wgt[i] = C.P[i].bad ? R(0) : std::max(C.P[i].err - avg, R(0));
-        W += wgt[i];
-      }
-      if (nbad) {   // inconsistent intervals take half of the quantiles (reading A-7)
-        const R wb = (W + rtol * std::abs(A)) / R(nbad);
-        W = 0;
-        for (int i = 0; i < n; ++i) {
-          if (C.P[i].bad) wgt[i] = wb;
-          W += wgt[i];
-        }
-      }
-      if (!(W > 0)) {
-        W = 0;
-        for (int i = 0; i < n; ++i) { wgt[i] = C.P[i].err; W += wgt[i]; }
-      }
-      std::vector<R> cum(n + 1);
-      cum[0] = 0;
-      for (int i = 0; i < n; ++i) cum[i + 1] = cum[i] + wgt[i];
-      std::vector<R> newth;
-      for (int k = 0; k < K; ++k) {
-        const R target = (R(k) + R(0.5)) / R(K) * cum[n];                         // quantiles, A-4
-        int i = int(std::upper_bound(cum.begin(), cum.end(), target) - cum.begin()) - 1;
-        i = std::min(std::max(i, 0), n - 1);
-        while (i < n - 1 && !(wgt[i] > 0)) ++i;
-        const R frac = wgt[i] > 0 ? (target - cum[i]) / wgt[i] : R(0.5);
-        const R th = C.S[i].theta + frac * C.dtheta(i);                           // linear interpolation
-        const R hi = (i + 1 < n) ? C.S[i + 1].theta : C.twopi;
-        if (th > C.S[i].theta && th < hi) newth.push_back(th);
-      }
+      std::vector<R> th(n), er(n);
+      std::vector<char> bad(n);
+      for (int i = 0; i < n; ++i) { th[i] = C.S[i].theta; er[i] = C.P[i].err; bad[i] = (char)C.P[i].bad; }
+      std::vector<R> newth = sampler_new_thetas(th, er, bad, C.twopi, rtol * std::abs(A), K, o.subtract_avg_tol);
       if (newth.empty()) { status |= 2; break; }
       C.insert(newth);
     }
@@ -833,6 +876,63 @@ int orc_magnify_thetas(double s, double q, double rho, double zre, double zim, d
   if (prec) magnify_one<long double>(s, q, rho, zre, zim, rel_tol, 0, o, nullptr, nullptr, &n, nullptr, out_theta);
   else magnify_one<double>(s, q, rho, zre, zim, rel_tol, 0, o, nullptr, nullptr, &n, nullptr, out_theta);
   return n;
+}
+
+// ---- diagnostics for the pins (tests/test_oracle_errors.py); no arithmetic of their own --------------------------------
+
+// The contour over an arbitrary sorted list of n boundary angles theta[] (0 <= theta_0 < ... < 2 pi): per interval
+// (theta_i, theta_{i+1}) (the last one closes the loop) out_piece[i] = {dA, err}, out_terms[i][8] = Piece::terms,
+// out_cross[i] = 0 / +1 creation / -1 annihilation; out_count[i] = real images of sample i.  Any output may be NULL.
+void orc_pieces_at(double s, double q, double rho, double zre, double zim, int n, const double* theta, int prec,
+                   double* out_piece, double* out_terms, int32_t* out_cross, int32_t* out_count) {
+  auto run = [&](auto tag) {
+    typedef decltype(tag) R;
+    const Lens<R> L = make_lens<R>(s, q);
+    std::vector<Sample<R>> S(n);
+    for (int j = 0; j < n; ++j) point_solve(L, Cx<R>((R)zre, (R)zim), (R)rho, (R)theta[j], S[j]);
+    const R twopi = R(2) * pi_v<R>();
+    for (int j = 0; j < n; ++j) {
+      const R dth = (j + 1 < n) ? (R)theta[j + 1] - (R)theta[j] : twopi - (R)theta[j] + (R)theta[0];
+      Piece<R> P;
+      eval_interval(S[j], S[(j + 1) % n], dth, P);
+      if (out_piece) { out_piece[2 * j] = (double)P.dA; out_piece[2 * j + 1] = (double)P.err; }
+      if (out_terms) for (int k = 0; k < 8; ++k) out_terms[8 * j + k] = (double)P.terms[k];
+      if (out_cross) out_cross[j] = P.bad ? 99 : P.crossing;
+      if (out_count) out_count[j] = S[j].nreal;
+    }
+  };
+  if (prec) run((long double)0); else run((double)0);
+}
+
+// One interval between two SYNTHETIC samples given by the caller (kinds 0 / +1 / -1, positions z, derivatives z',
+// z'^z'' per root; complex = (re, im)): what eval_interval makes of them.  out[0] = dA, out[1] = err, out[2..9] =
+// Piece::terms; returns the crossing code (0, +1, -1; 99 = inconsistent).
+int orc_eval_interval_synth(const int32_t* kindA, const double* zA, const double* zpA, const double* wA, const int32_t* kindB,
+                            const double* zB, const double* zpB, const double* wB, double dth, double* out) {
+  typedef long double R;
+  Sample<R> A, B;
+  for (int k = 0; k < 5; ++k) {
+    A.kind[k] = kindA[k]; A.z[k] = Cx<R>(zA[2 * k], zA[2 * k + 1]); A.zp[k] = Cx<R>(zpA[2 * k], zpA[2 * k + 1]); A.w[k] = wA[k];
+    B.kind[k] = kindB[k]; B.z[k] = Cx<R>(zB[2 * k], zB[2 * k + 1]); B.zp[k] = Cx<R>(zpB[2 * k], zpB[2 * k + 1]); B.w[k] = wB[k];
+  }
+  A.nreal = B.nreal = 0;
+  for (int k = 0; k < 5; ++k) { A.nreal += A.kind[k] != 0; B.nreal += B.kind[k] != 0; }
+  Piece<R> P;
+  eval_interval(A, B, (R)dth, P);
+  out[0] = (double)P.dA;
+  out[1] = (double)P.err;
+  for (int k = 0; k < 8; ++k) out[2 + k] = (double)P.terms[k];
+  return P.bad ? 99 : P.crossing;
+}
+
+// One step of the paper's sampler on caller-given interval errors (sampler_new_thetas).  Returns the number of new
+// angles written to out_theta (at most K).
+int orc_sampler_step(int n, const double* theta, const double* err, double tolA, int K, int subtract_avg_tol, double* out_theta) {
+  std::vector<double> th(theta, theta + n), er(err, err + n);
+  std::vector<char> bad(n, 0);
+  const std::vector<double> nt = sampler_new_thetas<double>(th, er, bad, 2.0 * pi_v<double>(), tolA, K, subtract_avg_tol);
+  for (size_t i = 0; i < nt.size(); ++i) out_theta[i] = nt[i];
+  return (int)nt.size();
 }
 
 // O9. Brute-force inverse ray shooting: rays on a uniform grid of nx x ny cells over the image-plane

@@ -104,8 +104,9 @@ def test_ray_shooting_agrees(s, q, rho, zeta, ncross):
 
 def test_fig2_topology_and_crossing_sign():
     """P-6 (tests/golden/fig2_topology.txt): exactly two crossings, one creation and one
-    annihilation; and the crossing correction carries the sign of DESIGN.md S-2 (with the other sign the
-    fixed-N error at N=256 is > 1e-3 instead of < 1e-4)."""
+    annihilation; with the crossing correction Eq.(11) the fixed-N value converges fast (without it, or with a flipped
+    sign, the N = 512 error is > 1e-4 instead of < 1.5e-5).  The sign itself is pinned, separately for creation and
+    annihilation, by the fold model in tests/test_oracle_errors.py."""
     rows = [l.split() for l in open(os.path.join(GOLD, "fig2_topology.txt")) if not l.startswith("#")]
     s, q, rho, zr, zi = map(float, rows[0])
     n_cross, n_closed, n_broken, n_pos, n_neg = map(int, rows[1])
@@ -123,7 +124,7 @@ def test_fig2_topology_and_crossing_sign():
     assert (r["kind"][0][cnt == 5] < 0).sum(axis=1).max() == n_neg
     truth = mu_ref(s, q, rho, complex(zr, zi))
     assert abs(r["mu"][0] - truth) < 1e-4 * truth
-    assert abs(api.images_fixed(wl, 512)["mu"][0] - truth) < 3e-5 * truth
+    assert abs(api.images_fixed(wl, 512)["mu"][0] - truth) < 1.5e-5 * truth
 
 
 def test_parabolic_correction_is_fourth_order():
@@ -166,16 +167,12 @@ def test_fig1_zoom_centre():
     cx, cy = map(float, rows[1])
     for sign in (-1, +1):
         zc = complex(zr, sign * zi)
-        th = np.linspace(0, 2 * np.pi, 400001)[:-1]
-        # coarse scan for 5-image samples with the extended-precision face
-        idx5 = [t for t in th[::40] if api.point(s, q, rho, zc, t, 1)["nreal"] == 5]
         fine = []
         lo = (2.6215 if sign < 0 else 2 * np.pi - 2.6240)
         for t in np.linspace(lo, lo + 0.0025, 2501):
             p = api.point(s, q, rho, zc, t, 1)
             if p["nreal"] == 5:
                 fine.append((t, p))
-        assert len(idx5) == 0 or True
         assert len(fine) > 10
         width = fine[-1][0] - fine[0][0]
         assert 1.0e-4 < width < 3.0e-4
@@ -197,7 +194,7 @@ def test_fig6_positions_are_smooth():
     a = api.magnify(wl, 1e-4, mode=0)
     b = api.magnify(wl, 1e-6, mode=1, prec=1)
     assert np.all(a["status"] & 1)
-    assert np.abs(a["mu"] / b["mu"] - 1).max() < 3e-4        # the estimate is not a strict bound (few x tol)
+    assert np.abs(a["mu"] / b["mu"] - 1).max() < 1e-4        # within the preset tolerance
     curve = b["mu"][2:]
     # no spike: second differences of the converged curve stay small against the curve's own range
     d2 = np.abs(np.diff(curve, 2))
@@ -210,7 +207,8 @@ def test_fig6_positions_are_smooth():
 
 def test_error_estimate_and_stop_rule():
     """when the paper-style sampler stops with E <= tol |A| the true error (vs the extended-precision
-    converged reference) is within a few tol; the cap returns value + estimate with status 2."""
+    converged reference) is within tol ("all the results are still within the preset relative tolerance"); the cap
+    returns value + estimate with status 2."""
     rng = np.random.default_rng(5)
     zs = 0.35 * (rng.uniform(-1, 1, 60) + 1j * rng.uniform(-1, 1, 60))
     wl = W.Workload("t", np.array([1.0]), np.array([0.1]), np.array([0.02]), np.zeros(60, np.int32),
@@ -221,8 +219,8 @@ def test_error_estimate_and_stop_rule():
         assert np.all(r["status"] & 1)
         assert np.all(r["err"] <= tol)
         rel = np.abs(r["mu"] / truth - 1)
-        assert rel.max() < 5 * tol, (tol, rel.max())
-        assert np.median(rel) < tol
+        assert rel.max() < tol, (tol, rel.max())
+        assert np.median(rel) < 0.1 * tol
     r = api.magnify(wl.subset([0, 1, 2]), 1e-12, mode=0, max_samples=512)
     assert np.all(r["status"] & 2) and np.all(r["nsamples"] <= 512) and np.all(r["nsamples"] > 512 - 64)
     assert np.all(np.isfinite(r["mu"])) and np.all(r["err"] > 1e-12)
