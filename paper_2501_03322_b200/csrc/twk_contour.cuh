@@ -522,16 +522,11 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth, double 
     const double dtt3 = dtt * dtt * dtt;
     const double corr = (wpl - wmi) * dtt3 * (1.0 / 24.0);              // Eq.(11)
     const double dd = dotp(d, ppl - pmi);
-    double chord, dAp, E2;
-    if (creation) {   // path z- -> z+, correction enters with '-' (S-2)
-      chord = 0.5 * wedge(zmi, d);
-      dAp = -corr;
-      E2 = 1.5 * fabs(dd - 2.0 * ad * sq) * dtt;                        // Eq.(18), reading E-5
-    } else {          // path z+ -> z-, correction enters with '+'
-      chord = -0.5 * wedge(zpl, d);
-      dAp = corr;
-      E2 = 1.5 * fabs(dd + 2.0 * ad * sq) * dtt;
-    }
+    // Eq.(11) enters as printed in both directions (S-2): the pair's path runs z- -> z+ at a creation and
+    // z+ -> z- at an annihilation; only the closing chord and the sign rule of E2 depend on the direction
+    const double dAp = corr;
+    const double chord = creation ? 0.5 * wedge(zmi, d) : -0.5 * wedge(zpl, d);
+    const double E2 = 1.5 * fabs(creation ? dd - 2.0 * ad * sq : dd + 2.0 * ad * sq) * dtt;   // Eq.(18), reading E-5
     P.crossing = creation ? 1 : -1;
     P.dA += chord + dAp;
     const double E1 = fabs(wpl + wmi) * dtt3 * (1.0 / 48.0);            // Eq.(18)
