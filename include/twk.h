@@ -43,7 +43,8 @@ extern "C" {
 #define TWK_ST_REPAIRED 4u   /* a sample's parity sum was not -1 and was repaired (reading G-5)        */
 #define TWK_ST_DOMAIN 8u     /* s, q outside the validated domain 0.1<=s<=10, q>=1e-9: still computed;   */
                              /* non-finite / non-positive s, q, rho or non-finite zeta: out_mu = NaN             */
-#define TWK_ST_NUMERIC 16u   /* a non-finite value appeared in the solve (degenerate quintic, zeta on a lens)    */
+#define TWK_ST_NUMERIC 16u   /* a boundary sample sat on a lens and was moved off it by 1e-14 s (reading B-1; mu is */
+                             /* finite and accurate), or a non-finite value appeared in the solve (mu = NaN)         */
 #define TWK_ST_SLOPE 32u     /* the slope detector re-judged a real image pair as ghosts (reading G-4) */
 #define TWK_ST_POINT 64u     /* point-source adequacy tests passed: out_mu = point-source magnification +   */
                              /* quadrupole term, no contour was integrated, out_nsamples = 0                        */
@@ -123,6 +124,28 @@ int twk_magnify_lightcurve(twk_ctx* ctx, size_t n_models, const double* s, const
 int twk_images_fixed(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
                      size_t n_sources, const int32_t* model_id, const double* zeta, int N, double* out_z,
                      int8_t* out_kind, int8_t* out_count, double* out_mu, double* out_err, void* stream);
+
+/* Diagnostics for the parity harness: fixed sampling with the solver of the ADAPTIVE kernels.  As twk_images_fixed, but
+ * every boundary sample is solved the way twk_magnify solves it: the point source at the
+ * source centre is solved once, its five roots and their first-order response predict the roots of every boundary
+ * sample, which are refined by Newton on the undeflated quintic, verified by Vieta's sums, recovered through Vieta's
+ * formulas when two chains merge, with the cold Laguerre solver as last resort.
+ *   out_diag   DEVICE uint32[4] or NULL: {point solves, Vieta recoveries, cold-solver fallbacks, lens-guard hits} */
+int twk_images_fixed_seeded(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                            size_t n_sources, const int32_t* model_id, const double* zeta, int N, double* out_z,
+                            int8_t* out_kind, int8_t* out_count, double* out_mu, double* out_err, uint32_t* out_diag,
+                            void* stream);
+
+/* Diagnostics for the parity harness: the sample records of the FIRST iteration (64 uniform samples theta_j = 2 pi j / 64,
+ * P:318) exactly as the stage-1 kernel of twk_magnify computes them (same kernel, a dump switched on).
+ *   out_records DEVICE double[n_sources][26][64]: element e of sample j of source i at [i][e][j]; per sample
+ *               e = 0..4 Re z, 5..9 Im z of slots 0..4 (slots 0,1 positive-parity images, 2,3,4 negative-parity images;
+ *               a sample with 3 real images keeps them in slots 0, 2, 3 and its ghost pair's positions in slots 1 and 4),
+ *               10..14 Re z', 15..19 Im z', 20..24 z'^z'' (real images only), 25 = (number of real images + 8 * flags)
+ *               as the raw bits of an int64.  Sources with invalid parameters are left untouched.
+ *   out_diag    DEVICE uint32[4] or NULL: as above */
+int twk_stage1_records(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho, size_t n_sources,
+                       const int32_t* model_id, const double* zeta, double* out_records, uint32_t* out_diag, void* stream);
 
 /* End-to-end convenience with HOST buffers (same meaning as twk_magnify): copies the inputs host->device into the
  * context's staging area, runs twk_magnify on `stream`, copies the outputs device->host and synchronises the

@@ -170,6 +170,7 @@ template <class R> struct Sample {
   int nreal;
   int repaired;       // parity repair fired (reading G-5)
   int slope;          // a real pair of this sample was re-judged as ghosts by the slope detector
+  int guard;          // the sample sat on a lens and was moved off it (reading B-1)
   int sweeps;
 };
 
@@ -179,7 +180,14 @@ void point_solve(const Lens<R>& L, const Cx<R>& zc, R rho, R theta, Sample<R>& S
   const Cx<R> e(std::cos(theta), std::sin(theta));
   S.zeta = zc + rho * e;
   S.dzeta = Cx<R>(0, 1) * rho * e;
-  const Cx<R> y = S.zeta - L.z2;
+  Cx<R> y = S.zeta - L.z2;
+  // B-1: a boundary point ON a lens (conj(y) = 0 or conj(y) = -s) makes c5 = 0: one root escapes to
+  // infinity and one sits on the pole of f.  The magnification is continuous there, so a point closer to a lens than
+  // 1e-14 s -- the rounding of zeta itself -- is moved to that distance (along the lens axis); status bit 16.
+  S.guard = 0;
+  const R dmin = R(1e-14) * L.s;
+  if (std::abs(y) < dmin) { y = Cx<R>(dmin, 0); S.guard = 1; }
+  if (std::abs(y + L.s) < dmin) { y = Cx<R>(-L.s + dmin, 0); S.guard = 1; }
   coeffs_eq6(y, L.s, L.m2, S.c);
   Cx<R> eta[5];
   S.sweeps = quintic_roots_dk(S.c, eta);
@@ -635,12 +643,14 @@ void magnify_one(double s, double q, double rho_, double zre, double zim, double
       C.insert(newth);
     }
   }
-  int rep = 0, slp = 0;
+  int rep = 0, slp = 0, grd = 0;
   for (const auto& smp : C.S) {
     rep |= smp.repaired;
     slp |= smp.slope;
+    grd |= smp.guard;
   }
   if (rep || nbad) status |= 4;
+  if (grd) status |= 16;
   if (slp) status |= 32;
   if (out_mu) *out_mu = (double)(A / (pi_v<R>() * C.rho * C.rho));
   if (out_err) *out_err = (double)(E / std::abs(A));

@@ -17,7 +17,7 @@ _lib = None
 TWK_ST_CONVERGED, TWK_ST_CAP, TWK_ST_REPAIRED, TWK_ST_DOMAIN, TWK_ST_NUMERIC, TWK_ST_SLOPE, TWK_ST_POINT = 1, 2, 4, 8, 16, 32, 64
 
 SYMBOLS = ["twk_default_options", "twk_create", "twk_destroy", "twk_workspace_bytes", "twk_magnify", "twk_magnify_lightcurve",
-           "twk_images_fixed",
+           "twk_images_fixed", "twk_images_fixed_seeded", "twk_stage1_records",
            "twk_magnify_host", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_strerror", "twk_version"]
 
 
@@ -53,6 +53,8 @@ def lib():
         L.twk_magnify_lightcurve.argtypes = [vp, sz, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
         L.twk_magnify_host.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
         L.twk_images_fixed.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, vp]
+        L.twk_images_fixed_seeded.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
+        L.twk_stage1_records.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, vp, vp, vp]
         L.twk_last_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int), vp]
         L.twk_enable_stage_timing.argtypes = [vp, i32]
         L.twk_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
@@ -186,6 +188,33 @@ class Context:
                "twk_images_fixed")
         return dict(z=z, kind=kind, count=count, mu=mu, err=err)
 
+    def twk_images_fixed_seeded(self, s, q, rho, zeta, N, model_id=None, stream=None):
+        """As twk_images_fixed with the adaptive kernels' solver; adds diag = uint32[4] {solves, recoveries, cold, guard}."""
+        import torch
+        n = int(zeta.shape[0])
+        dev = zeta.device
+        z = torch.empty((n, N, 5, 2), dtype=torch.float64, device=dev)
+        kind = torch.empty((n, N, 5), dtype=torch.int8, device=dev)
+        count = torch.empty((n, N), dtype=torch.int8, device=dev)
+        mu = torch.empty(n, dtype=torch.float64, device=dev)
+        err = torch.empty(n, dtype=torch.float64, device=dev)
+        diag = torch.zeros(4, dtype=torch.int32, device=dev)
+        _check(lib().twk_images_fixed_seeded(self._h, int(s.shape[0]), _ptr(s), _ptr(q), _ptr(rho), n, _ptr(model_id),
+                                             _ptr(zeta), int(N), _ptr(z), _ptr(kind), _ptr(count), _ptr(mu), _ptr(err),
+                                             _ptr(diag), _stream_ptr(stream)), "twk_images_fixed_seeded")
+        return dict(z=z, kind=kind, count=count, mu=mu, err=err, diag=diag)
+
+    def twk_stage1_records(self, s, q, rho, zeta, model_id=None, stream=None):
+        """The first-iteration records of the stage-1 kernel: dict(records float64[n, 26, 64], diag int32[4])."""
+        import torch
+        n = int(zeta.shape[0])
+        dev = zeta.device
+        rec = torch.zeros((n, 26, 64), dtype=torch.float64, device=dev)
+        diag = torch.zeros(4, dtype=torch.int32, device=dev)
+        _check(lib().twk_stage1_records(self._h, int(s.shape[0]), _ptr(s), _ptr(q), _ptr(rho), n, _ptr(model_id), _ptr(zeta),
+                                        _ptr(rec), _ptr(diag), _stream_ptr(stream)), "twk_stage1_records")
+        return dict(records=rec, diag=diag)
+
     # -- host-buffer call (end to end) -----------------------------------------------------------------------------
     def twk_magnify_host(self, s, q, rho, zeta, model_id=None, rel_tol=1e-4, out=None, stream=None):
         """Host buffers: numpy arrays or (pinned) CPU torch tensors, float64 / int32, C-contiguous.  Synchronous.
@@ -230,9 +259,27 @@ class Context:
         r = self.twk_magnify(d["s"], d["q"], d["rho"], d["zeta"], d["model_id"], wl.rel_tol if rel_tol is None else rel_tol)
         return {k: v.cpu().numpy() for k, v in r.items()}
 
-    def images_fixed_workload(self, wl, N=None):
+    def images_fixed_workload(self, wl, N=None, seeded=False):
         d = self.upload(wl)
-        r = self.twk_images_fixed(d["s"], d["q"], d["rho"], d["zeta"], int(N or wl.fixed_n), d["model_id"])
+        f = self.twk_images_fixed_seeded if seeded else self.twk_images_fixed
+        r = f(d["s"], d["q"], d["rho"], d["zeta"], int(N or wl.fixed_n), d["model_id"])
         o = {k: v.cpu().numpy() for k, v in r.items()}
         o["z"] = o["z"][..., 0] + 1j * o["z"][..., 1]
         return o
+
+    def stage1_records_workload(self, wl):
+        """Stage-1 records unpacked like images_fixed_workload (N = 64): z complex[n, 64, 5], kind int8[n, 64, 5] (by record
+        slot: a 3-image sample holds its ghosts in slots 1 and 4), count int8[n, 64], flags int[n, 64], diag."""
+        d = self.upload(wl)
+        r = self.twk_stage1_records(d["s"], d["q"], d["rho"], d["zeta"], d["model_id"])
+        rec = r["records"].cpu().numpy()                                  # [n, 26, 64]
+        z = np.moveaxis(rec[:, 0:5, :] + 1j * rec[:, 5:10, :], 1, 2)      # [n, 64, 5]
+        code = np.ascontiguousarray(rec[:, 25, :]).view(np.int64)
+        count = (code & 7).astype(np.int8)
+        kind = np.empty(z.shape, np.int8)
+        kind[...] = np.array([1, 1, -1, -1, -1], np.int8)
+        three = count == 3
+        kind[three, 1] = 0
+        kind[three, 4] = 0
+        return dict(z=z, kind=kind, count=count, flags=(code >> 3).astype(np.int32), diag=r["diag"].cpu().numpy(),
+                    zp=np.moveaxis(rec[:, 10:15, :] + 1j * rec[:, 15:20, :], 1, 2), w=np.moveaxis(rec[:, 20:25, :], 1, 2))

@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
 
     // ---- outputs / hand-over ------------------------------------------------------------------------------------
     const int rep = __syncthreads_or(flags & kPointRepaired);
-    const int nonf = __syncthreads_or(flags & kPointNonFinite);
+    const int nonf = __syncthreads_or(flags & (kPointNonFinite | kPointGuard));
     const int slp = __syncthreads_or(flags & kPointSlope);
     if (t == 0) {
       if (exhausted && !p.final_stage) {

@@ -310,9 +310,10 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
   return TWK_OK;
 }
 
-int twk_images_fixed(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
-                     size_t n_sources, const int32_t* model_id, const double* zeta, int N, double* out_z,
-                     int8_t* out_kind, int8_t* out_count, double* out_mu, double* out_err, void* stream_) {
+static int images_fixed_impl(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                             size_t n_sources, const int32_t* model_id, const double* zeta, int N, double* out_z,
+                             int8_t* out_kind, int8_t* out_count, double* out_mu, double* out_err, bool seeded,
+                             uint32_t* out_diag, void* stream_) {
   const int rc = check_batch(ctx, n_models, s, q, rho, n_sources, model_id, zeta);
   if (rc != TWK_OK) return rc;
   if (n_sources == 0) return TWK_OK;
@@ -320,10 +321,61 @@ int twk_images_fixed(twk_ctx* ctx, size_t n_models, const double* s, const doubl
   cudaStream_t stream = (cudaStream_t)stream_;
   twk::Batch b{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame,
                nullptr, nullptr, nullptr, nullptr, nullptr};
-  const size_t smem = (size_t)(twk::kRecDoubles * kFixedTile + 2 * twk::kRecDoubles + 2 * (kFixedTile / 32)) * 8;
+  const size_t smem = (size_t)(twk::kRecDoubles * kFixedTile + 2 * twk::kRecDoubles + 2 * (kFixedTile / 32) + 32) * 8;
   const long long resident = (long long)ctx->sms * 8;
   const int grid = (int)((long long)n_sources < resident ? (long long)n_sources : resident);
-  twk::fixed_kernel<kFixedTile><<<grid, kFixedTile, smem, stream>>>(b, N, out_z, out_kind, out_count, out_mu, out_err);
+  if (seeded) {
+    if (out_diag) TWK_CUDA(cudaMemsetAsync(out_diag, 0, 4 * sizeof(uint32_t), stream));
+    twk::fixed_kernel<kFixedTile, true><<<grid, kFixedTile, smem, stream>>>(b, N, out_z, out_kind, out_count, out_mu, out_err, out_diag);
+  } else {
+    twk::fixed_kernel<kFixedTile, false><<<grid, kFixedTile, smem, stream>>>(b, N, out_z, out_kind, out_count, out_mu, out_err, nullptr);
+  }
+  ctx->last_launches = 1;
+  TWK_CUDA(cudaGetLastError());
+  return TWK_OK;
+}
+
+int twk_images_fixed(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                     size_t n_sources, const int32_t* model_id, const double* zeta, int N, double* out_z,
+                     int8_t* out_kind, int8_t* out_count, double* out_mu, double* out_err, void* stream_) {
+  return images_fixed_impl(ctx, n_models, s, q, rho, n_sources, model_id, zeta, N, out_z, out_kind, out_count, out_mu, out_err,
+                           false, nullptr, stream_);
+}
+
+int twk_images_fixed_seeded(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                            size_t n_sources, const int32_t* model_id, const double* zeta, int N, double* out_z,
+                            int8_t* out_kind, int8_t* out_count, double* out_mu, double* out_err, uint32_t* out_diag,
+                            void* stream_) {
+  return images_fixed_impl(ctx, n_models, s, q, rho, n_sources, model_id, zeta, N, out_z, out_kind, out_count, out_mu, out_err,
+                           true, out_diag, stream_);
+}
+
+int twk_stage1_records(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho, size_t n_sources,
+                       const int32_t* model_id, const double* zeta, double* out_records, uint32_t* out_diag, void* stream_) {
+  const int rc = check_batch(ctx, n_models, s, q, rho, n_sources, model_id, zeta);
+  if (rc != TWK_OK) return rc;
+  if (n_sources == 0) return TWK_OK;
+  if (!out_records) return TWK_EINVAL;
+  cudaStream_t stream = (cudaStream_t)stream_;
+  int* counters = reinterpret_cast<int*>(ctx->ws + ctx->lay.counters);
+  TWK_CUDA(cudaMemsetAsync(counters, 0, 64, stream));
+  if (out_diag) TWK_CUDA(cudaMemsetAsync(out_diag, 0, 4 * sizeof(uint32_t), stream));
+  twk::Stage1Args a{};
+  a.b = twk::Batch{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame,
+                   nullptr, nullptr, nullptr, nullptr, nullptr};
+  a.tol = 1.0;                 // irrelevant: nothing is handed on (final_stage), nothing is written but the records
+  a.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
+  a.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
+  a.ps_test = 0;
+  a.final_stage = 1;
+  a.cursor = counters + 0;
+  a.list = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list1);
+  a.list_count = counters + 1;
+  a.handoff = nullptr;
+  a.handoff_slots = 0;
+  a.dump = out_records;
+  a.diag = out_diag;
+  launch_stage1(ctx->sms, (long long)n_sources, a, stream);
   ctx->last_launches = 1;
   TWK_CUDA(cudaGetLastError());
   return TWK_OK;

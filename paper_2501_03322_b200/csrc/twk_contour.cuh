@@ -16,7 +16,7 @@ namespace twk {
 //   [10..14] Re z'    z' = dz/dtheta, Eq.(10) (conj on f' restored)
 //   [15..19] Im z'
 //   [20..24] z'^z''   Eq.(10) (division by J restored)
-//   [25]    nreal (3 or 5) + 8 * point flags (kPointRepaired | kPointNonFinite | kPointSlope), an integer kept as raw bits
+//   [25]    nreal (3 or 5) + 8 * point flags (kPoint*), an integer kept as raw bits
 // In shared memory the record is a column of a [26][TILE] array (stride = TILE, conflict-free); in the global
 // arena it is 26 contiguous doubles (stride = 1, 208 B).
 // ------------------------------------------------------------------------------------------------------------
@@ -60,6 +60,20 @@ struct RecRef {
 constexpr int kPointRepaired = 1;   // parity sum was not -1 and was repaired (G-5)
 constexpr int kPointSlope = 4;      // a real pair was re-judged as ghosts by the slope detector
 constexpr int kPointNonFinite = 2;  // a root or a derived quantity is not finite
+constexpr int kPointGuard = 8;      // the sample sat on a lens and was moved off it (reading B-1)
+constexpr int kPointRecovered = 16; // diagnostics: the seeded solve went through its Vieta recovery
+constexpr int kPointCold = 32;      // diagnostics: the cold solver was used (no seeds, or the seeded solve failed)
+
+// B-1: a boundary point ON a lens (conj(y) = 0 or conj(y) = -s) makes c5 = 0: one root escapes to infinity
+// and one sits on the pole of f.  The magnification is continuous there, so a point closer to a lens than 1e-14 s --
+// the rounding of zeta itself -- is moved to that distance along the lens axis.  Returns true when it fired.
+TWK_HD bool lens_guard(cd& y, double s) {
+  const double dmin = 1e-14 * s;
+  bool fired = false;
+  if (norm2(y) < dmin * dmin) { y = mk(dmin, 0.0); fired = true; }
+  if (norm2(mk(y.x + s, y.y)) < dmin * dmin) { y = mk(-s + dmin, 0.0); fired = true; }
+  return fired;
+}
 
 // ------------------------------------------------------------------------------------------------------------
 // a1 + a2 + a3 + a4 + a5: one boundary point source.
@@ -73,11 +87,14 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
                           RecRef rec, double* out_z, int8_t* out_kind, int8_t* out_count) {
   const cd zeta = mk(fma(rho, cs, zc.x), fma(rho, sn, zc.y));
   const cd dzeta = mk(-rho * sn, rho * cs);                     // zeta' = i rho e^{i theta}
-  const cd y = mk(zeta.x - L.z2, zeta.y);
+  cd y = mk(zeta.x - L.z2, zeta.y);
+  const bool guarded = lens_guard(y, L.s);
   cd c[6], eta[5];
   coeffs_eq6(y, L.s, L.m2, c);
-  bool solved = false;
-  if (seeds) {
+  int solved = 0;
+  // next to a lens (closer than 1e-8 s) one root runs off towards infinity and one onto the pole: left to the cold solver
+  const bool near_lens = fmin(norm2(y), norm2(mk(y.x + L.s, y.y))) < 1e-16 * L.s * L.s;
+  if (seeds && !near_lens) {
     const double dx = rho * cs, dy = rho * sn;                  // delta
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
@@ -89,6 +106,7 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     }
     solved = quintic_roots_seeded(c, eta, seeds[30 * seed_stride] != 0.0);
   }
+  int flags = (guarded ? kPointGuard : 0) | (solved == 2 ? kPointRecovered : 0) | (solved ? 0 : kPointCold);
   if (!solved) {
     TWK_COUNT(cold_solve);
     Coef6 C;
@@ -145,7 +163,7 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     npos += (kind[k] > 0);
   }
   // parity sum must be -1.  Repair by flipping the smallest-|J| image of the over-represented parity.
-  int flags = finite ? 0 : kPointNonFinite;
+  flags |= finite ? 0 : kPointNonFinite;
   const int want = (nreal - 1) >> 1;
   for (int guard = 0; guard < 5 && npos != want; ++guard) {
     const int over = (npos > want) ? 1 : -1;
@@ -167,7 +185,8 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     const cd z = mk(eta[k].x + L.z2, eta[k].y);
     if (out_z) { out_z[2 * k] = z.x; out_z[2 * k + 1] = z.y; }
     if (out_kind) out_kind[k] = (int8_t)kind[k];
-    if (kind[k] != 0) {
+    // (slots stay inside the record whatever the kinds are: with non-finite J every kind is -1)
+    if (kind[k] != 0 && (kind[k] > 0 ? sp < 2 : sm < 5)) {
       const int slot = (kind[k] > 0) ? sp++ : sm++;
       const double invJ = rcp(J[k]);
       // z' = (zeta' - conj(f') conj(zeta')) / J                       Eq.(10), repaired (E-2)
@@ -194,13 +213,6 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   return flags;
 }
 
-TWK_HD int point_solve(const Lens& L, cd zc, double rho, double theta, RecRef rec, double* out_z, int8_t* out_kind,
-                       int8_t* out_count) {
-  double sn, cs;
-  sincos(theta, &sn, &cs);
-  return point_solve_cs(L, zc, rho, cs, sn, nullptr, 0, rec, out_z, out_kind, out_count);
-}
-
 // Seed block of one source (kSeedDoubles doubles, element e at seeds[e * stride]):
 //   [0..4] Re eta_k, [5..9] Im eta_k   the five planet-frame roots of the point source at the source CENTRE (cold solve)
 //   [10..14] Re A_k, [15..19] Im A_k, [20..24] Re B_k, [25..29] Im B_k
@@ -219,7 +231,8 @@ constexpr int kSeedDoubles = 31;
 TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int stride) {
   cd c[6], eta[5];
   double dmin2_all = 1e300;
-  const cd y = mk(zc.x - L.z2, zc.y);
+  cd y = mk(zc.x - L.z2, zc.y);
+  lens_guard(y, L.s);   // a source CENTRE on a lens is an ordinary input (the disk covers the lens)
   coeffs_eq6(y, L.s, L.m2, c);
   {
     Coef6 C;
@@ -285,7 +298,8 @@ constexpr double kPsGhost = 0.1;   // reading N1-c
 
 TWK_HD bool point_source_adequate(const Lens& L, cd zc, double rho, const double* seeds, int stride, double tol, double& mu,
                                   double& qrel) {
-  const cd y = mk(zc.x - L.z2, zc.y);
+  cd y = mk(zc.x - L.z2, zc.y);
+  lens_guard(y, L.s);
   cd eta[5], g[5], f[5], Res[5];
   double R2[5];
 #pragma unroll

@@ -270,7 +270,7 @@ TWK_NOINLINE Roots5 quintic_roots_cold(Coef6 C) {
 // converged after 10 sweeps, the three or four good distinct roots fix the others through Vieta's formulas
 // (sum of roots = -c4/c5, product = -c0/c5: one missing root directly, two as the roots of a quadratic); these
 // are polished by the same Newton sweeps and the verification is repeated.
-// Returns false when that fails too; the caller then falls back to the cold solver quintic_roots().
+// Returns 0 when that fails too; the caller then falls back to the cold solver quintic_roots().
 // r[] holds the seeds on entry and the roots on exit.
 // Two converged chains are the same root when they agree to 1e-6 of their size (RELATIVE: next to a planet of
 // q = 1e-9 two distinct roots can be 1e-9 apart in absolute terms while the other roots are of order one).
@@ -354,7 +354,8 @@ TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev) {
   return conv;
 }
 
-TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product) {
+// Returns 0 = failed (use the cold solver), 1 = solved, 2 = solved after the Vieta recovery.
+TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product) {
   double prev[5];
 #pragma unroll
   for (int k = 0; k < 5; ++k) prev[k] = 0.0;
@@ -377,13 +378,20 @@ TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_produc
         // flagged by centre_seeds (two roots closer than 1e-6 of the scale: next to a q = 1e-9 planet two chains on
         // one of two tiny neighbouring roots change the sum by 1e-9 of its scale, below this test), their product
         // (relative)
-        const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
-        bool ok = abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale;
-        if (check_product) {
+        // (a root that has run off towards infinity -- a sample next to a lens -- must not hide a duplicate among the
+        // others: the tolerance follows the OTHER four roots, plus the rounding of the largest one)
+        const double a0 = abs1(r[0]), a1 = abs1(r[1]), a2 = abs1(r[2]), a3 = abs1(r[3]), a4 = abs1(r[4]);
+        const double big = fmax(fmax(fmax(a0, a1), fmax(a2, a3)), a4);
+        const double scale = (a0 + a1) + (a2 + a3) + a4 - big;
+        bool ok = abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale + 1e-14 * big;
+        // ... and ALWAYS the product: the sum alone is blind to two duplicated chains whose errors cancel (a sample at a
+        // symmetric point: equal masses, zeta = 0), and to a duplicate among roots 1e-9 of the scale apart
+        {
           const cd prod = ((r[0] * r[1]) * (r[2] * r[3])) * r[4];
           ok = ok && abs1(prod * c[5] + c[0]) <= 1e-9 * abs1(c[0]);          // prod = -c0/c5
         }
-        if (ok) return true;
+        (void)check_product;
+        if (ok) return recovered ? 2 : 1;
       }
       if (recovered) break;
       recovered = true;
@@ -409,7 +417,7 @@ TWK_HD bool quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_produc
     }
   }
   TWK_COUNT(fail_iter);
-  return false;
+  return 0;
 }
 
 }  // namespace twk

@@ -63,8 +63,10 @@ __device__ __forceinline__ SourceParams load_source(const Batch& b, long long sr
     P.zc = mk(b.zeta[2 * src], b.zeta[2 * src + 1]);
   }
   P.rho = rho;
-  P.valid = (s > 0.0) && (q > 0.0) && (rho > 0.0) && isfinite(s) && isfinite(q) && isfinite(rho) && isfinite(P.zc.x) &&
-            isfinite(P.zc.y) && m_in >= 0 && m_in < b.n_models;
+  // finite, positive, and of a magnitude whose fourth powers stay finite (the coefficients are quartic in zeta and s)
+  constexpr double kHuge = 1e50;
+  P.valid = (s > 0.0) && (q > 0.0) && (rho > 0.0) && (s < kHuge) && (q < kHuge) && (rho < kHuge) && (fabs(P.zc.x) < kHuge) &&
+            (fabs(P.zc.y) < kHuge) && (s > 1.0 / kHuge) && (q > 1.0 / kHuge) && m_in >= 0 && m_in < b.n_models;
   P.status = (P.valid && s >= 0.1 && s <= 10.0 && q >= 1e-9) ? 0u : 8u;
   P.L = make_lens(P.valid ? s : 1.0, P.valid ? q : 1.0);
   if (b.frame == 1) P.zc.x += P.L.z2 - P.L.s;   // z1 = -q s / (1 + q) = z2 - s  (reading F-1)
@@ -93,15 +95,18 @@ __device__ __forceinline__ void block_sum2(double& a, double& b, double* scratch
 // Fixed-sampling mode.  TILE threads; records of one tile of samples in shared memory ([26][TILE]); the interval
 // (j-1 -> j) is evaluated by the thread of sample j, with the previous tile's last record carried over.
 // ------------------------------------------------------------------------------------------------------------
-template <int TILE>
+// SEEDED: every sample is solved as the adaptive kernels solve it -- centre_seeds() once per source, then the seeded
+// Newton solve with Vieta recovery and the cold solver as fallback (twk_images_fixed_seeded; diag counts the events).
+template <int TILE, bool SEEDED>
 __global__ void __launch_bounds__(TILE) fixed_kernel(Batch b, int N, double* __restrict__ out_z, int8_t* __restrict__ out_kind,
                                                      int8_t* __restrict__ out_count, double* __restrict__ out_mu,
-                                                     double* __restrict__ out_err) {
+                                                     double* __restrict__ out_err, unsigned* __restrict__ diag) {
   extern __shared__ double sm[];
   double* rec = sm;                          // [26][TILE]
   double* carry = rec + kRecDoubles * TILE;  // [26] last record of the previous tile
   double* first = carry + kRecDoubles;       // [26] record of sample 0
   double* red = first + kRecDoubles;         // [2 * TILE/32]
+  double* seeds = red + 2 * (TILE / 32);     // [31] seed block of the source (SEEDED)
   const int t = threadIdx.x;
   for (long long src = blockIdx.x; src < b.n_sources; src += gridDim.x) {
     const SourceParams S = load_source(b, src);
@@ -114,13 +119,30 @@ __global__ void __launch_bounds__(TILE) fixed_kernel(Batch b, int N, double* __r
     }
     double accA = 0.0, accE = 0.0;
     const double dth = kTwoPi / double(N);
+    if (SEEDED) {
+      if (t == 0) centre_seeds(S.L, S.zc, S.rho, seeds, 1);
+      __syncthreads();
+    }
     for (int base = 0; base < N; base += TILE) {
       const int j = base + t;
       const RecRef mine{rec + t, TILE};
+      int flags = 0;
       if (j < N) {
         const size_t o = (size_t)src * N + j;
-        point_solve(S.L, S.zc, S.rho, kTwoPi * double(j) / double(N), mine, out_z ? out_z + o * 10 : nullptr,
-                    out_kind ? out_kind + o * 5 : nullptr, out_count ? out_count + o : nullptr);
+        double sn, cs;
+        sincos(kTwoPi * double(j) / double(N), &sn, &cs);
+        flags = point_solve_cs(S.L, S.zc, S.rho, cs, sn, SEEDED ? seeds : nullptr, 1, mine, out_z ? out_z + o * 10 : nullptr,
+                               out_kind ? out_kind + o * 5 : nullptr, out_count ? out_count + o : nullptr);
+      }
+      if (SEEDED && diag) {
+        const unsigned act = __ballot_sync(0xffffffffu, j < N), rcv = __ballot_sync(0xffffffffu, flags & kPointRecovered),
+                       cold = __ballot_sync(0xffffffffu, flags & kPointCold), grd = __ballot_sync(0xffffffffu, flags & kPointGuard);
+        if ((t & 31) == 0) {
+          if (act) atomicAdd(diag + 0, (unsigned)__popc(act));
+          if (rcv) atomicAdd(diag + 1, (unsigned)__popc(rcv));
+          if (cold) atomicAdd(diag + 2, (unsigned)__popc(cold));
+          if (grd) atomicAdd(diag + 3, (unsigned)__popc(grd));
+        }
       }
       __syncthreads();
       if (j < N && j >= 1) {

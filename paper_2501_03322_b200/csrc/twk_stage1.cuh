@@ -32,10 +32,13 @@ struct Stage1Args {
   int* list_count;       // entries of `list` (zeroed before launch)
   double* handoff;       // [handoff_slots][kHandDoubles] first-iteration state of worklist entries < handoff_slots
   long long handoff_slots;
-  double* out_mu;
+  double* out_mu;        // may be null (twk_stage1_records)
   double* out_err;       // may be null
   int32_t* out_nsamples; // may be null
   uint32_t* out_status;  // may be null
+  // diagnostics (twk_stage1_records): the 64 records of every source as this kernel computed them, and event counts
+  double* dump;          // [n_sources][26][64] or null
+  unsigned* diag;        // [4]: point solves, Vieta recoveries, cold solves, lens-guard hits; or null
 };
 
 constexpr int kS1ParamRows = 8;   // s, m1, m2, z2, Re zc, Im zc, rho, status|valid
@@ -128,6 +131,16 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
       const cd zc = mk(prm[4 * kS1Group + i], prm[5 * kS1Group + i]);
       const double rho = prm[6 * kS1Group + i];
       int flags = point_solve_cs(L, zc, rho, cs, sn, seeds + i, kS1Group, mine, nullptr, nullptr, nullptr);
+      if (p.diag) {
+        const unsigned rec = __ballot_sync(0xffffffffu, flags & kPointRecovered), cold = __ballot_sync(0xffffffffu, flags & kPointCold),
+                       grd = __ballot_sync(0xffffffffu, flags & kPointGuard);
+        if ((t & 31) == 0) {
+          atomicAdd(p.diag + 0, 32u);
+          if (rec) atomicAdd(p.diag + 1, (unsigned)__popc(rec));
+          if (cold) atomicAdd(p.diag + 2, (unsigned)__popc(cold));
+          if (grd) atomicAdd(p.diag + 3, (unsigned)__popc(grd));
+        }
+      }
       __syncthreads();                                   // the 64 records are complete
       Piece P;
       double A, E;
@@ -171,6 +184,11 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
         }
         __syncthreads();
       }
+      if (p.dump) {
+        double* d = p.dump + (size_t)(base + i) * (kRecDoubles * kThreads);
+#pragma unroll 1
+        for (int e = 0; e < kRecDoubles; ++e) d[e * kThreads + t] = mine.at(e);
+      }
       // every thread holds A, E and the flags: the decisions are uniform
       const bool finite = isfinite(A) && isfinite(E);
       const bool pend = finite && !(E <= p.tol * fabs(A)) && !p.final_stage;   // stop rule P:272
@@ -198,7 +216,7 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
         else if (E <= p.tol * fabs(A)) status |= 1u;               // stop rule P:272
         else if (p.final_stage) status |= 2u;                       // cap P:326
         if (flags & kPointRepaired) status |= 4u;
-        if (flags & kPointNonFinite) status |= 16u;
+        if (flags & (kPointNonFinite | kPointGuard)) status |= 16u;
         if (flags & kPointSlope) status |= 32u;
         res_mu[i] = A * rcp(kPi * rho * rho);
         res_err[i] = E * rcp(fabs(A));
@@ -211,7 +229,7 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
     // ---- phase 3: coalesced results -----------------------------------------------------------------------------------
     {
       const long long src = base + t;
-      if (t < G && src < n && !res_pend[t]) {
+      if (t < G && src < n && !res_pend[t] && p.out_mu) {
         p.out_mu[src] = res_mu[t];
         if (p.out_err) p.out_err[src] = res_err[t];
         if (p.out_nsamples) p.out_nsamples[src] = res_ns[t];

@@ -49,6 +49,76 @@ def check_fixed(ctx, wl, N):
     return g, o
 
 
+def compare_samples(g, o, what):
+    """Element by element: counts and kinds identical, all five positions within POS_TOL after matching."""
+    assert np.array_equal(g["count"], o["count"]), what
+    idx = match_roots(g["z"], o["z"])
+    assert np.all(np.sort(idx, axis=-1) == np.arange(5)), "root matching is not a permutation"
+    zg = np.take_along_axis(g["z"], idx, axis=-1)
+    kg = np.take_along_axis(g["kind"], idx, axis=-1)
+    assert np.array_equal(kg, o["kind"]), what
+    rel = np.abs(zg - o["z"]) / np.maximum(1.0, np.abs(o["z"]))
+    assert rel.max() <= POS_TOL, (what, rel.max())
+    return rel.max()
+
+
+SEEDED_CASES = [("config1", {}, 256), ("fig2", {}, 256), ("fig1", {}, 256), ("fig2", {}, 100), ("fig1", {}, 301),
+                ("config3", dict(n_models=400, n_epochs=10), 64), ("config5", dict(n=3000), 64), ("lowq_sweep", {}, 64),
+                ("domain_corners", {}, 64), ("fig5_map", dict(case="close", nx=48, ny=34), 64),
+                ("fig7_grid", dict(n_side=4), 64)]
+
+
+@pytest.mark.parametrize("name,kw,N", SEEDED_CASES)
+def test_seeded_solver_positions(ctx, name, kw, N):
+    """north_star: "GPU image positions must match the oracle's to 1e-10 relative and the image counts must match
+    exactly" -- for the solver the TIMED kernels run: centre roots + first-order prediction -> Newton on the undeflated
+    quintic -> Vieta verification / recovery -> cold fallback (twk_images_fixed_seeded runs exactly that per sample)."""
+    wl = W.get(name, **kw)
+    g = ctx.images_fixed_workload(wl, N, seeded=True)
+    o = api.images_fixed(wl, N, prec=0)
+    compare_samples(g, o, name)
+    assert np.abs(g["mu"] / o["mu"] - 1).max() < 1e-8
+    assert g["diag"][0] == wl.n_sources * N
+
+
+def test_seeded_solver_branches_ran(ctx):
+    """The Vieta recovery and the cold fallback of the seeded solve are exercised by the low-q workloads (merged chains
+    next to a q ~ 1e-9 planet) and by caustic-crossing boundaries -- counted by the library, and the positions of those
+    very samples are inside the comparison above."""
+    tot = np.zeros(4, np.int64)
+    for name, kw, N in SEEDED_CASES:
+        d = ctx.images_fixed_workload(W.get(name, **kw), N, seeded=True)["diag"].astype(np.int64)
+        tot += d
+        if name in ("config3", "config5"):
+            assert d[1] + d[2] < 0.02 * d[0], (name, d)     # ... and on the BASELINE batches they are the exception
+    assert tot[1] > 100 and tot[2] > 10, tot          # recoveries, cold fallbacks
+
+
+@pytest.mark.parametrize("name,kw", [("config1", {}), ("fig2", {}), ("fig1", {}), ("config2", {}),
+                                     ("config3", dict(n_models=400, n_epochs=10)), ("config5", dict(n=3000)),
+                                     ("lowq_sweep", {}), ("domain_corners", {}), ("fig7_grid", dict(n_side=4))])
+def test_stage1_kernel_records(ctx, name, kw):
+    """The same bar on what the stage-1 kernel of twk_magnify itself computed (twk_stage1_records: the timed kernel with
+    its record dump switched on): the 64 first-iteration samples of every source -- five positions, kinds, counts --
+    against the oracle at N = 64; z' and z'^z'' of the real images against the oracle's too."""
+    wl = W.get(name, **kw)
+    g = ctx.stage1_records_workload(wl)
+    o = api.images_fixed(wl, 64, prec=0)
+    compare_samples(g, o, name)
+    assert g["diag"][0] == wl.n_sources * 64
+    if name in ("fig2", "config1"):
+        # derivatives of the real images, sample by sample against the oracle's point face
+        m = int(wl.model_id[0])
+        for j in (0, 17, 40):
+            p = api.point(wl.s[m], wl.q[m], wl.rho[m], complex(*wl.zeta[0]), 2 * np.pi * j / 64, 0)
+            for k in range(5):
+                if g["kind"][0, j, k] == 0:
+                    continue
+                ko = int(np.argmin(np.abs(p["z"] - g["z"][0, j, k])))
+                assert abs(g["zp"][0, j, k] - p["zp"][ko]) <= 1e-9 * abs(p["zp"][ko])
+                assert abs(g["w"][0, j, k] - p["w"][ko]) <= 1e-8 * abs(p["w"][ko]) + 1e-18
+
+
 def test_fixed_config1(ctx):
     wl = W.config1()
     g, o = check_fixed(ctx, wl, 256)
@@ -364,16 +434,41 @@ def test_edge_cases(ctx):
     g = c3.magnify_workload(wl, 1e-12)
     assert (int(g["status"][0]) & 2) and g["nsamples"][0] == 64
     c3.close()
-    # a boundary sample exactly on a lens (degenerate quintic): must not hang or crash; flagged or finite
-    q0, s0 = 0.5, 1.0
-    z2 = s0 / (1 + q0)
-    r = ctx.twk_magnify(f([s0]), f([q0]), f([0.25]), f([[z2 - 0.25, 0.0]]), None, 1e-4)
-    st = int(r["status"].cpu().numpy()[0])
-    assert (st & 16) or np.isfinite(r["mu"].cpu().numpy()[0])
+    # huge but finite inputs: rejected like non-finite ones (the coefficients are quartic in them)
+    r = ctx.twk_magnify(f([1.0, 1.0]), f([0.1, 0.1]), f([0.01, 1e200]), f([[1e200, 0.0], [0.1, 0.1]]), None, 1e-4)
+    assert np.all(np.isnan(r["mu"].cpu().numpy())) and np.all(r["status"].cpu().numpy() == 8)
     # too many sources for the context
     with pytest.raises(P.TwkError):
         small = P.Context(4)
         small.twk_magnify(f([1.0]), f([0.1]), f([0.01]), f([[0.1, 0.1]] * 5), None, 1e-4)
+
+
+def test_boundary_sample_on_a_lens(ctx):
+    """Reading B-1: a boundary sample EXACTLY on a lens (c5 = 0: a root at infinity and one on the pole) is moved off it
+    by 1e-14 s.  The magnification is finite and continuous there: it equals the oracle's (same rule) and the value of
+    sources shifted by 1e-9, and carries status bit 16 next to 'converged'.  Round numbers that gridded maps hit."""
+    cases = [(1.0, 1.0, 0.25, 0.25 + 0j),        # theta = 0 lands on z2 = 0.5
+             (1.0, 1.0, 0.25, 0.5 - 0.25j),      # theta = pi/2 lands on z2
+             (1.0, 1.0, 0.25, -0.25 + 0j),       # theta = pi lands on z1 = -0.5
+             (0.8, 0.25, 0.125, -0.285 + 0j),    # theta = 0 lands on z1 = -0.16
+             (1.0, 1.0, 0.5, 0.0 + 0j),          # theta = 0 on z2 AND theta = pi on z1
+             (1.0, 1.0, 0.25, 0.25 + 0j)]
+    for s, q, rho, zc in cases:
+        z = np.array([zc, zc + 1e-9, zc - 1e-9j, zc + 3e-9 + 2e-9j])
+        wl = W.Workload("b1", np.array([s]), np.array([q]), np.array([rho]), np.zeros(4, np.int32),
+                        np.stack([z.real, z.imag], 1).copy(), 1e-6)
+        for tol in (1e-4, 1e-6):
+            g = ctx.magnify_workload(wl, tol)
+            st = g["status"].astype(np.uint32)
+            assert np.all(np.isfinite(g["mu"])) and np.all(st & 1)
+            assert st[0] & 16 and not np.any(st[1:] & 16)
+            assert np.abs(g["mu"][0] / g["mu"][1:] - 1).max() < max(2e-7, 0.5 * tol)
+        ref = api.magnify(wl, 1e-6, mode=1)
+        assert ref["status"][0] & 16
+        assert np.abs(g["mu"] / ref["mu"] - 1).max() <= MU_TOL
+        # and in fixed mode the guarded sample has the oracle's positions
+        compare_samples(ctx.images_fixed_workload(wl.subset([0]), 64), api.images_fixed(wl.subset([0]), 64), "B-1 cold")
+        compare_samples(ctx.stage1_records_workload(wl.subset([0])), api.images_fixed(wl.subset([0]), 64), "B-1 stage 1")
 
 
 def test_host_buffer_entry_point(ctx):

@@ -437,3 +437,33 @@ def test_parity_repair_flips_the_smallest_jacobian():
             solid = real & (np.abs(p["J"]) > 1e-4)
             assert np.all(p["kind"][solid] == np.sign(p["J"][solid])), (s, q, zeta, p["J"], p["kind"])
     assert fired >= 10, fired
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# B-1: a boundary sample exactly on a lens
+# ---------------------------------------------------------------------------------------------------------------------
+def test_boundary_sample_on_a_lens_is_continuous():
+    """Reading B-1: with a boundary sample EXACTLY on a lens the quintic loses its leading coefficient (c5 = -conj(y) v_c
+    = 0, Eq.(6)); the oracle moves such a sample off the lens by 1e-14 s.  The magnification is a continuous function of
+    the source position there, so the result must agree with sources shifted by ~1e-9 in any direction (which never
+    trigger the rule) to the accuracy asked for, and carry status bit 16."""
+    cases = [(1.0, 1.0, 0.25, 0.25 + 0j), (1.0, 1.0, 0.25, 0.5 - 0.25j), (1.0, 1.0, 0.25, -0.25 + 0j),
+             (0.8, 0.25, 0.125, -0.285 + 0j), (1.0, 0.5, 0.25, 1 / 1.5 - 0.25 + 0j)]
+    for s, q, rho, zc in cases:
+        z = np.array([zc, zc + 1e-9, zc - 1e-9j, zc + 3e-9 + 2e-9j])
+        wl = W.Workload("b1", np.array([s]), np.array([q]), np.array([rho]), np.zeros(4, np.int32),
+                        np.stack([z.real, z.imag], 1).copy(), 1e-6)
+        for mode in (0, 1):
+            r = api.magnify(wl, 1e-6, mode=mode)
+            assert np.all(np.isfinite(r["mu"])) and np.all(r["status"] & 1)
+            assert r["status"][0] & 16 and not np.any(r["status"][1:] & 16)
+            assert np.abs(r["mu"][0] / r["mu"][1:] - 1).max() < 1e-6
+        # the sample on the lens: two of the five roots are the degenerate ones (on the pole, run away), both ghosts
+        hit = 0
+        for th in (0.0, np.pi / 2, np.pi, 1.5 * np.pi):
+            zj = zc + rho * complex(np.cos(th), np.sin(th))
+            if min(abs(zj - s / (1 + q)), abs(zj + q * s / (1 + q))) < 1e-15:
+                p = api.point(s, q, rho, zc, th, 0)
+                assert p["nreal"] == 3 and np.abs(p["z"][p["kind"] == 0]).max() > 1e12
+                hit += 1
+        assert hit >= 1
