@@ -160,10 +160,10 @@ int twk_last_stats(twk_ctx* ctx, int64_t* n_stage2, int64_t* n_stage3, int* n_la
 
 /* Per-stage device timing of twk_magnify for measurement: when enabled, CUDA events are recorded on the call's
  * stream around each stage.  twk_last_stage_ms waits for the last recorded event and writes the durations (ms)
- * of {stage-1 kernel, stage-2 kernel, stage-3 kernel} of the last twk_magnify on this context (0 for absent
- * stages) into ms3[3]. */
+ * of {stage-0 (centre solves), stage-1, stage-2, stage-3 kernel} of the last twk_magnify on this context (0 for
+ * absent stages) into ms4[4]. */
 int twk_enable_stage_timing(twk_ctx* ctx, int on);
-int twk_last_stage_ms(twk_ctx* ctx, float* ms3);
+int twk_last_stage_ms(twk_ctx* ctx, float* ms4);
 
 /* FP64 FMA throughput probe used for the ALU roofline denominator: runs `iters` dependent-chain DFMAs per thread
  * (8 independent chains per thread, a full persistent grid) and returns the measured TFLOP/s (2 flop per DFMA) in

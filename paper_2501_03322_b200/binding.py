@@ -243,9 +243,9 @@ class Context:
         _check(lib().twk_enable_stage_timing(self._h, 1 if on else 0), "twk_enable_stage_timing")
 
     def twk_last_stage_ms(self):
-        ms = (C.c_float * 3)()
+        ms = (C.c_float * 4)()
         _check(lib().twk_last_stage_ms(self._h, ms), "twk_last_stage_ms")
-        return dict(stage1=ms[0], stage2=ms[1], stage3=ms[2])
+        return dict(stage0=ms[0], stage1=ms[1], stage2=ms[2], stage3=ms[3])
 
     # -- convenience over a workloads.Workload ------------------------------------------------------------------------
     def upload(self, wl, device="cuda"):

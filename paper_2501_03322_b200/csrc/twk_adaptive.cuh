@@ -29,6 +29,7 @@ struct AdaptArgs {
   int32_t* next_list;    // stage 2 only: sources that need stage 3 ...
   int* next_count;       // ... appended with atomicAdd
   double* arena;         // stages 2/3: gridDim.x * cap records of kRecDoubles doubles
+  const double* seeds;   // [kSeedDoubles][n_sources] seed blocks written by stage 0
   const double* handoff; // stage 2: hand-over arena written by stage 1 (null: recompute the first iteration)
   long long handoff_slots;   // worklist entries < handoff_slots have a hand-over slot
   double* out_mu;
@@ -106,7 +107,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
       flags |= recref(t).point_flags();
       n = kThreads;
     } else {      // not handed over: the loop below starts by inserting the 64 uniform samples into the empty list
-      if (t == 0) centre_seeds(S.L, S.zc, S.rho, seeds, 1);
+      if (t < kSeedDoubles) seeds[t] = p.seeds[(size_t)t * (size_t)p.b.n_sources + (size_t)src];
     }
     uint32_t status = S.status;
     bool exhausted = false, slope_seen = false;

@@ -47,7 +47,7 @@ size_t handoff_slots(const twk_options& o, size_t max_sources) {
 }
 
 struct Layout {
-  size_t counters, list1, list2, handoff, arena, total;
+  size_t counters, list1, list2, seeds, handoff, arena, total;
   size_t slots;
 };
 Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
@@ -58,6 +58,7 @@ Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
   L.counters = off; off += 256;
   L.list1 = off;    off += align256(max_sources * 4);
   L.list2 = off;    off += align256(max_sources * 4);
+  L.seeds = off;    off += align256(max_sources * twk::kSeedDoubles * 8);
   L.handoff = off;  off += align256(L.slots * twk::kHandDoubles * 8);
   L.arena = off;    off += align256(P.arena_doubles * 8);
   L.total = off;
@@ -110,7 +111,7 @@ struct twk_ctx {
   size_t stage_bytes;
   int last_launches;
   int timing;            // record CUDA events around every stage (twk_enable_stage_timing)
-  cudaEvent_t ev[5];     // start, after stage 1, after stage 2, after stage 3
+  cudaEvent_t ev[5];     // start, after stage 0, after stage 1, after stage 2, after stage 3
   int ev_used;           // number of events recorded by the last call
 };
 
@@ -256,6 +257,16 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     if (ctx->timing && ctx->ev_used < 5) cudaEventRecord(ctx->ev[ctx->ev_used++], stream);
   };
   mark();
+  // ---- stage 0: the point source at every source centre -> seed blocks --------------------------------------------
+  double* seeds = reinterpret_cast<double*>(ctx->ws + ctx->lay.seeds);
+  a.seeds = seeds;
+  {
+    const long long want = ((long long)n_sources + twk::kS0Threads - 1) / twk::kS0Threads;
+    const long long cap = (long long)ctx->sms * 16;
+    twk::seeds_kernel<<<(int)(want < cap ? want : cap), twk::kS0Threads, 0, stream>>>(batch, seeds);
+    ++launches;
+  }
+  mark();
   // ---- stage 1: every source, 64 samples, groups of 64 sources per CTA, everything in shared memory ----------------
   {
     twk::Stage1Args a1{};
@@ -265,6 +276,7 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a1.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
     a1.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
     a1.final_stage = P.cap2 ? 0 : 1;
+    a1.seeds = seeds;
     a1.cursor = counters + 0;
     a1.list = list1;
     a1.list_count = counters + 1;
@@ -363,6 +375,13 @@ int twk_stage1_records(twk_ctx* ctx, size_t n_models, const double* s, const dou
   twk::Stage1Args a{};
   a.b = twk::Batch{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame,
                    nullptr, nullptr, nullptr, nullptr, nullptr};
+  {
+    double* seeds = reinterpret_cast<double*>(ctx->ws + ctx->lay.seeds);
+    const long long want = ((long long)n_sources + twk::kS0Threads - 1) / twk::kS0Threads;
+    const long long cap = (long long)ctx->sms * 16;
+    twk::seeds_kernel<<<(int)(want < cap ? want : cap), twk::kS0Threads, 0, stream>>>(a.b, seeds);
+    a.seeds = seeds;
+  }
   a.tol = 1.0;                 // irrelevant: nothing is handed on (final_stage), nothing is written but the records
   a.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
   a.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
@@ -450,12 +469,12 @@ int twk_enable_stage_timing(twk_ctx* ctx, int on) {
   return TWK_OK;
 }
 
-int twk_last_stage_ms(twk_ctx* ctx, float* ms3) {
-  if (!ctx || !ms3) return TWK_EINVAL;
-  for (int i = 0; i < 3; ++i) ms3[i] = 0.0f;
+int twk_last_stage_ms(twk_ctx* ctx, float* ms4) {
+  if (!ctx || !ms4) return TWK_EINVAL;
+  for (int i = 0; i < 4; ++i) ms4[i] = 0.0f;
   if (!ctx->timing || ctx->ev_used < 2) return TWK_EINVAL;
   TWK_CUDA(cudaEventSynchronize(ctx->ev[ctx->ev_used - 1]));
-  for (int i = 0; i + 1 < ctx->ev_used && i < 3; ++i) TWK_CUDA(cudaEventElapsedTime(&ms3[i], ctx->ev[i], ctx->ev[i + 1]));
+  for (int i = 0; i + 1 < ctx->ev_used && i < 4; ++i) TWK_CUDA(cudaEventElapsedTime(&ms4[i], ctx->ev[i], ctx->ev[i + 1]));
   return TWK_OK;
 }
 

@@ -88,12 +88,14 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   const cd zeta = mk(fma(rho, cs, zc.x), fma(rho, sn, zc.y));
   const cd dzeta = mk(-rho * sn, rho * cs);                     // zeta' = i rho e^{i theta}
   cd y = mk(zeta.x - L.z2, zeta.y);
-  const bool guarded = lens_guard(y, L.s);
+  // next to a lens (closer than 1e-8 s) one root runs off towards infinity and one onto the pole: such a sample is left
+  // to the cold solver; ON the lens it is moved off it first (B-1)
+  const bool near_lens = fmin(norm2(y), norm2(mk(y.x + L.s, y.y))) < 1e-16 * L.s * L.s;
+  bool guarded = false;
+  if (near_lens) guarded = lens_guard(y, L.s);
   cd c[6], eta[5];
   coeffs_eq6(y, L.s, L.m2, c);
   int solved = 0;
-  // next to a lens (closer than 1e-8 s) one root runs off towards infinity and one onto the pole: left to the cold solver
-  const bool near_lens = fmin(norm2(y), norm2(mk(y.x + L.s, y.y))) < 1e-16 * L.s * L.s;
   if (seeds && !near_lens) {
     const double dx = rho * cs, dy = rho * sn;                  // delta
 #pragma unroll
@@ -137,22 +139,21 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   }
   // a5: residual detector, 2-cycle reading (G-1): the two largest-|R| roots (ia, ib) are a ghost pair iff
   // R_ia = eta_ib - eta_ia and R_ib = eta_ia - eta_ib ("a pair of ghost images with opposite residuals").
-  int ia = 0;
+  // (running maxima in scalars: no dynamically indexed array, everything stays in registers)
+  int ia = 0, ib = -1;
+  double mA = R2[0], mB = -1.0;
+  cd eA = eta[0], rA = Res[0], eB = eta[0], rB = Res[0];
 #pragma unroll
-  for (int k = 1; k < 5; ++k)
-    if (R2[k] > R2[ia]) ia = k;
-  int ib = (ia == 0) ? 1 : 0;
-#pragma unroll
-  for (int k = 0; k < 5; ++k)
-    if (k != ia && R2[k] > R2[ib]) ib = k;
-  cd eA = eta[0], eB = eta[0], rA = Res[0], rB = Res[0];
-#pragma unroll
-  for (int k = 0; k < 5; ++k) {
-    if (k == ia) { eA = eta[k]; rA = Res[k]; }
-    if (k == ib) { eB = eta[k]; rB = Res[k]; }
+  for (int k = 1; k < 5; ++k) {
+    if (R2[k] > mA) {          // new largest: the old largest becomes the second
+      mB = mA; ib = ia; eB = eA; rB = rA;
+      mA = R2[k]; ia = k; eA = eta[k]; rA = Res[k];
+    } else if (R2[k] > mB) {
+      mB = R2[k]; ib = k; eB = eta[k]; rB = Res[k];
+    }
   }
   const cd dab = eB - eA;
-  const bool ghost = norm2(rA - dab) < norm2(rA) && norm2(rB + dab) < norm2(rB);
+  const bool ghost = norm2(rA - dab) < mA && norm2(rB + dab) < mB;
   int kind[5];
   int nreal = 0, npos = 0;
 #pragma unroll
@@ -228,7 +229,10 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
 // a quarter of the distance to the nearest other root (next to a caustic 1/J blows up); otherwise A = B = 0.
 constexpr int kSeedDoubles = 31;
 
-TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int stride) {
+// Element e goes to seeds[e * stride] (stride > 0) or, for the [kSeedDoubles][n] workspace layout, to seeds[e * wide]
+// (stride == 0).
+TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int stride, long long wide = 0) {
+  const size_t st = stride > 0 ? (size_t)stride : (size_t)wide;
   cd c[6], eta[5];
   double dmin2_all = 1e300;
   cd y = mk(zc.x - L.z2, zc.y);
@@ -265,15 +269,15 @@ TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int st
       B = mk(0.0, 0.0);
     }
     dmin2_all = fmin(dmin2_all, dmin2);
-    seeds[k * stride] = eta[k].x;
-    seeds[(5 + k) * stride] = eta[k].y;
-    seeds[(10 + k) * stride] = A.x;
-    seeds[(15 + k) * stride] = A.y;
-    seeds[(20 + k) * stride] = B.x;
-    seeds[(25 + k) * stride] = B.y;
+    seeds[k * st] = eta[k].x;
+    seeds[(5 + k) * st] = eta[k].y;
+    seeds[(10 + k) * st] = A.x;
+    seeds[(15 + k) * st] = A.y;
+    seeds[(20 + k) * st] = B.x;
+    seeds[(25 + k) * st] = B.y;
   }
   const double scale = abs1(eta[0]) + abs1(eta[1]) + abs1(eta[2]) + abs1(eta[3]) + abs1(eta[4]);
-  seeds[30 * stride] = (dmin2_all < 1e-12 * scale * scale) ? 1.0 : 0.0;
+  seeds[30 * st] = (dmin2_all < 1e-12 * scale * scale) ? 1.0 : 0.0;
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -313,22 +317,21 @@ TWK_HD bool point_source_adequate(const Lens& L, cd zc, double rho, const double
     R2[k] = norm2(Res[k]);
   }
   // residual detector, as in point_solve_cs
-  int ia = 0;
+  // (running maxima in scalars: no dynamically indexed array, everything stays in registers)
+  int ia = 0, ib = -1;
+  double mA = R2[0], mB = -1.0;
+  cd eA = eta[0], rA = Res[0], eB = eta[0], rB = Res[0];
 #pragma unroll
-  for (int k = 1; k < 5; ++k)
-    if (R2[k] > R2[ia]) ia = k;
-  int ib = (ia == 0) ? 1 : 0;
-#pragma unroll
-  for (int k = 0; k < 5; ++k)
-    if (k != ia && R2[k] > R2[ib]) ib = k;
-  cd eA = eta[0], eB = eta[0], rA = Res[0], rB = Res[0];
-#pragma unroll
-  for (int k = 0; k < 5; ++k) {
-    if (k == ia) { eA = eta[k]; rA = Res[k]; }
-    if (k == ib) { eB = eta[k]; rB = Res[k]; }
+  for (int k = 1; k < 5; ++k) {
+    if (R2[k] > mA) {          // new largest: the old largest becomes the second
+      mB = mA; ib = ia; eB = eA; rB = rA;
+      mA = R2[k]; ia = k; eA = eta[k]; rA = Res[k];
+    } else if (R2[k] > mB) {
+      mB = R2[k]; ib = k; eB = eta[k]; rB = Res[k];
+    }
   }
   const cd dab = eB - eA;
-  const bool ghost = norm2(rA - dab) < norm2(rA) && norm2(rB + dab) < norm2(rB);
+  const bool ghost = norm2(rA - dab) < mA && norm2(rB + dab) < mB;
   double A = 0.0, Q = 0.0, Qabs = 0.0;
   int npos = 0, nreal = 0;
   bool ok = true;

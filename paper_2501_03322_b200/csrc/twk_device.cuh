@@ -155,7 +155,7 @@ TWK_HD void coeffs_eq6(cd y, double s, double m2, cd c[6]) {
 // ------------------------------------------------------------------------------------------------------------
 constexpr double kEps = 2.220446049250313e-16;
 #ifndef TWK_STOP_FACTOR
-#define TWK_STOP_FACTOR 0.125   // Newton stop rule: predicted next step <= TWK_STOP_FACTOR * eps * |root|
+#define TWK_STOP_FACTOR 450.0   // Newton stop rule: predicted next step <= TWK_STOP_FACTOR * eps * |root| = 1e-13 |root|
 #endif
 
 template <int N>
@@ -262,8 +262,8 @@ TWK_NOINLINE Roots5 quintic_roots_cold(Coef6 C) {
 // started from predictions of the roots (centre_seeds() in twk_contour.cuh).  Roots of a polynomial are continuous
 // in its coefficients, so ghosts can be followed like real images.
 // Stop rule per root: Newton converges quadratically, |dx_{n+1}| ~ K |dx_n|^2 with K ~ |dx_n| / |dx_{n-1}|^2, so
-// the step AFTER the one just taken would be ~ |dx_n|^3 / |dx_{n-1}|^2; once that is below eps/8 |r| the root is
-// converged and the confirming evaluation is skipped.  From the third iteration on the residual is also compared
+// the step AFTER the one just taken would be ~ |dx_n|^3 / |dx_{n-1}|^2; once that is below 1e-13 |r| (three orders
+// inside the 1e-10 position bar) the root is converged and the confirming evaluation is skipped.  From the third iteration on the residual is also compared
 // with the rounding floor of its own evaluation (ill-conditioned roots next to a caustic stall there).
 // Verification: all five converged and distinct (Vieta: sum of roots = -c4/c5).
 // Recovery (at most once per solve): when two chains ran into the same root, or up to two chains have not
@@ -378,14 +378,11 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
         // flagged by centre_seeds (two roots closer than 1e-6 of the scale: next to a q = 1e-9 planet two chains on
         // one of two tiny neighbouring roots change the sum by 1e-9 of its scale, below this test), their product
         // (relative)
-        // (a root that has run off towards infinity -- a sample next to a lens -- must not hide a duplicate among the
-        // others: the tolerance follows the OTHER four roots, plus the rounding of the largest one)
-        const double a0 = abs1(r[0]), a1 = abs1(r[1]), a2 = abs1(r[2]), a3 = abs1(r[3]), a4 = abs1(r[4]);
-        const double big = fmax(fmax(fmax(a0, a1), fmax(a2, a3)), a4);
-        const double scale = (a0 + a1) + (a2 + a3) + a4 - big;
-        bool ok = abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale + 1e-14 * big;
-        // ... and ALWAYS the product: the sum alone is blind to two duplicated chains whose errors cancel (a sample at a
-        // symmetric point: equal masses, zeta = 0), and to a duplicate among roots 1e-9 of the scale apart
+        const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
+        bool ok = abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale;
+        // ... and ALWAYS the product (relative): the sum alone is blind to two duplicated chains whose errors cancel (a
+        // sample at a symmetric point: equal masses, zeta = 0), to a duplicate among roots 1e-9 of the scale apart, and
+        // to any duplicate when one root has run off towards infinity (a sample next to a lens)
         {
           const cd prod = ((r[0] * r[1]) * (r[2] * r[3])) * r[4];
           ok = ok && abs1(prod * c[5] + c[0]) <= 1e-9 * abs1(c[0]);          // prod = -c0/c5
@@ -410,10 +407,21 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
         }
       done = S.done;
     }
+    // one step of every unfinished root; the root is moved through scalars (no dynamic indexing: r[] and prev[] stay
+    // in registers), one copy of the step's code
 #pragma unroll 1
     for (int k = 0; k < 5; ++k) {
       if (done & (1u << k)) continue;
-      if (newton_step<true>(c, r[k], prev[k])) done |= 1u << k;
+      cd x = r[0];
+      double pv = prev[0];
+#pragma unroll
+      for (int j = 1; j < 5; ++j)
+        if (j == k) { x = r[j]; pv = prev[j]; }
+      const bool cv = newton_step<true>(c, x, pv);
+#pragma unroll
+      for (int j = 0; j < 5; ++j)
+        if (j == k) { r[j] = x; prev[j] = pv; }
+      if (cv) done |= 1u << k;
     }
   }
   TWK_COUNT(fail_iter);

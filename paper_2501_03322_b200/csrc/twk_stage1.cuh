@@ -1,9 +1,8 @@
 // twk_stage1.cuh -- stage 1 of twk_magnify: the first iteration (64 uniform boundary samples) of EVERY source.
 //
 // One 64-thread CTA takes a group of up to 64 consecutive sources from an atomic cursor:
-//   phase 1  thread i cold-solves the point source at the CENTRE of source i (Laguerre + deflation): its five
-//            planet-frame roots and their first-order response to a source displacement are the seeds of that
-//            source's boundary samples (centre_seeds(), twk_contour.cuh);
+//   phase 1  thread i loads the parameters and the seed block of source i (stage 0: the five planet-frame roots of the
+//            point source at the source's CENTRE and their first-order response to a source displacement);
 //   phase 2  for each source of the group: thread t solves boundary sample t by seeded Newton on the undeflated
 //            quintic (verified; cold fallback), writes its record to shared memory, evaluates interval (t, t+1),
 //            block-reduces area and error and applies the stop rule.  An unfinished source is appended to
@@ -19,6 +18,22 @@
 
 namespace twk {
 
+// ------------------------------------------------------------------------------------------------------------
+// Stage 0: the point source at the CENTRE of every source (one thread per source): cold solve (Laguerre + deflation)
+// and the first-order response of the five roots to a source displacement = the seed block of that source's boundary
+// samples (centre_seeds(), twk_contour.cuh), written to the workspace as [kSeedDoubles][n_sources] so that stage 1 reads
+// it coalesced.  A kernel of its own: the ~6 k instructions of the cold solver stay out of the instruction stream of
+// the stage-1 loop (which fills the 32 KB instruction cache by itself).
+// ------------------------------------------------------------------------------------------------------------
+constexpr int kS0Threads = 128;
+__global__ void __launch_bounds__(kS0Threads) seeds_kernel(Batch b, double* __restrict__ seeds) {
+  const long long n = b.n_sources;
+  for (long long src = (long long)blockIdx.x * kS0Threads + threadIdx.x; src < n; src += (long long)gridDim.x * kS0Threads) {
+    const SourceParams S = load_source(b, src);
+    if (S.valid) centre_seeds(S.L, S.zc, S.rho, seeds + src, (int)0, n);
+  }
+}
+
 struct Stage1Args {
   Batch b;
   double tol;
@@ -27,6 +42,7 @@ struct Stage1Args {
   int ps_test;           // N1: point-source adequacy tests in front of the contour path (twk_options.point_source_test)
   int group;             // sources per group, 1..64 (smaller for small batches: more CTAs get work)
   int final_stage;       // 1: there is no refinement stage (max_samples < 128): cap status instead of pending
+  const double* seeds;   // [kSeedDoubles][n_sources] seed blocks written by stage 0
   int* cursor;           // group fetch counter (zeroed before launch)
   int32_t* list;         // [n_sources] a9: worklist of unfinished sources, appended in completion order
   int* list_count;       // entries of `list` (zeroed before launch)
@@ -95,7 +111,8 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
         prm[6 * kS1Group + t] = S.rho;
         int code = (int)S.status | (S.valid ? 256 : 0);
         if (S.valid) {
-          centre_seeds(S.L, S.zc, S.rho, seeds + t, kS1Group);
+#pragma unroll 1
+          for (int e = 0; e < kSeedDoubles; ++e) seeds[e * kS1Group + t] = p.seeds[(size_t)e * (size_t)n + (size_t)src];
           if (p.ps_test) {   // N1: quadrupole + ghost-image tests; adequate -> no contour for this source
             const PsResult r = point_source_adequate_cold(S.L, S.zc, S.rho, seeds + t, kS1Group, p.tol);
             if (r.ok) {
