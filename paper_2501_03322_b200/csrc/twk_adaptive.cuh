@@ -44,6 +44,8 @@ __host__ __device__ inline size_t adaptive_smem_bytes(int cap) {
   return doubles * 8 + ints * 4 + (size_t)cap * 2;
 }
 
+// 6 CTAs per SM (168 registers): measured 4 / 5 / 6 / 8 CTAs per SM on configs 3 and 5: 9.4 / 9.3 / 8.6 / 8.8 ms and
+// 7.6 / 7.4 / 6.7 / 7.0 ms -- the kernel is latency-bound and wants warps, but at 128 registers it spills
 __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   extern __shared__ double sm[];
   const int cap = p.cap;

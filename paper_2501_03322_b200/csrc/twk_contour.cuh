@@ -121,7 +121,7 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
 
   // a4: f', f'', residual, Jacobian in the planet frame (z2 - z = -eta, z1 - z = -s - eta; both are frame
   // invariant)
-  cd fp[5], fpp[5], Res[5];
+  cd fp[5], a3[5], b3[5], Res[5];
   double J[5], R2[5];
   bool finite = true;
 #pragma unroll
@@ -131,7 +131,8 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     const cd a2 = a * a, b2 = b * b;
     const cd f = L.m1 * a + L.m2 * b;                    // Eq.(7)
     fp[k] = L.m1 * a2 + L.m2 * b2;
-    fpp[k] = 2.0 * (L.m1 * (a2 * a) + L.m2 * (b2 * b));
+    a3[k] = a2 * a;                                      // f'' is finished below, for the real images only
+    b3[k] = b2 * b;
     Res[k] = mk(y.x - eta[k].x - f.x, y.y - eta[k].y + f.y);   // Eq.(12): y - eta - conj(f)
     J[k] = 1.0 - norm2(fp[k]);                           // Eq.(7)
     R2[k] = norm2(Res[k]);
@@ -194,7 +195,8 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
       const cd t = conj(fp[k]) * conj(dzeta);
       const cd zp = mk((dzeta.x - t.x) * invJ, (dzeta.y - t.y) * invJ);
       // z'^z'' = (rho^2 + Im[z'^2 zeta' f'']) / J                     Eq.(10), repaired (E-3)
-      const cd u = (zp * zp) * (dzeta * fpp[k]);
+      const cd fpp = 2.0 * (L.m1 * a3[k] + L.m2 * b3[k]);
+      const cd u = (zp * zp) * (dzeta * fpp);
       const double w = fma(rho, rho, u.y) * invJ;
       rec.at(kZX + slot) = z.x;
       rec.at(kZY + slot) = z.y;

@@ -331,9 +331,9 @@ TWK_NOINLINE SeededState seeded_recover(cd c0, cd c5, cd tot, SeededState S) {
 template <bool kFloor>
 TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev) {
   TWK_COUNT(newton_eval);
-  cd p = c[5], d = mk(0.0, 0.0);
+  cd p = cfma(c[5], x, c[4]), d = c[5];      // Horner for p and p', first step peeled (p' starts from c5, not from 0)
 #pragma unroll
-  for (int i = 4; i >= 0; --i) {
+  for (int i = 3; i >= 0; --i) {
     d = cfma(d, x, p);
     p = cfma(p, x, c[i]);
   }
@@ -363,6 +363,7 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
   unsigned done = 0;
   // sweeps 0 and 1: every root needs them (the stop rule wants two steps), so all five chains run unconditionally
   // and interleave (instruction-level parallelism); a step on an already converged root is harmless
+  // (a rolled loop of two sweeps: one copy of the five interleaved chains keeps the hot loop inside the instruction cache)
 #pragma unroll 1
   for (int it = 0; it < 2; ++it) {
     unsigned dn = 0;

@@ -59,7 +59,7 @@ struct Stage1Args {
 
 constexpr int kS1ParamRows = 8;   // s, m1, m2, z2, Re zc, Im zc, rho, status|valid
 constexpr int kS1Group = 64;      // sources per group at most (one centre solve per thread)
-constexpr int kS1CtasPerSM = 6;   // 12 warps per SM at <= 168 registers
+constexpr int kS1CtasPerSM = 6;   // 12 warps per SM at <= 168 registers (measured 3 / 4 / 5 / 6 CTAs: 42.8 / 34.9 / 32.5 / 29.8 ms)   // 12 warps per SM at <= 168 registers
 
 __host__ __device__ constexpr size_t stage1_smem_bytes() {
   return (size_t)(kRecDoubles * kThreads + kSeedDoubles * kS1Group + kS1ParamRows * kS1Group + 2 * kS1Group + 2 * 4) * 8 +
