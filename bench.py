@@ -1,18 +1,31 @@
 #!/usr/bin/env python
-"""bench.py -- finite-source magnifications/s of the twk hot path on BASELINE config 3 (Measurement).
+"""bench.py -- finite-source magnifications/s of the twk hot path (Measurement).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl twk|reference] [--workload config3]
 
-A "step" is one pass of the whole hot path (stage 1 -> stage 2 -> stage 3 of twk_magnify, all SURVEY 8(a) rows) over
-one batch of synthetic input: config 3 = 4,096 seeded lens models x 1,000 epochs = 4,096,000 source positions at
-relative tolerance 1e-4.  `value` = magnifications/s with inputs resident in HBM; `e2e` = the same through
-twk_magnify_host with pinned HOST buffers (H2D + D2H inside the timed region).  Rank 0 prints ONE JSON line.
-For N > 1 every rank runs its own batch (different seed): independent problems, no collective -> "weak" scaling.
+A "step" is one pass of the whole hot path (stage 0 -> 1 -> 2 -> 3 of twk_magnify, all SURVEY 8(a) rows) over one batch
+of synthetic input.  Headline workload: BASELINE config 3 = 4,096 seeded lens models x 1,000 epochs = 4,096,000 source
+positions at relative tolerance 1e-4.  `value` = magnifications/s with inputs resident in HBM; `e2e` = the same through
+twk_magnify_host with pinned HOST buffers (H2D + D2H inside the timed region).  Rank 0 prints ONE JSON line.  For N > 1
+every rank runs its own batch (different seed): independent problems, no collective -> "weak" scaling.
 --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+
+Roofline inputs are not constants of this file: the executed FP64 instructions (DFMA / DMUL / DADD) and the DRAM bytes of
+every kernel launch come from profiles/r02_counts.json, which `--parse-ncu` writes from an ncu pass over
+`bench.py --profile-pass` (one step of every workload below) and which carries the hash of the CUDA sources it was
+measured on.  When that hash is not the hash compiled into the loaded library (twk_version()), the counts are stale and
+`roofline.achieved` is withheld (null) instead of being wrong.
+
+Other modes (not part of the driver's contract):
+  --profile-pass         one untimed step of every workload (what the ncu counting pass runs)
+  --parse-ncu FILE.csv   turn the ncu --csv log of that pass into profiles/r02_counts.json
+  --scaling              time twk_magnify against the number of sources (the paper's Fig.8 question) and
+                         write profiles/r02_scaling.csv
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -27,14 +40,15 @@ sys.path.insert(0, ROOT)
 
 METRIC = "finite-source magnifications/sec at rel. acc 1e-4"
 UNIT = "magnifications/s"
-# FP64 flop per boundary point (a1-a7: sample, coefficients, solve, lens quantities, ghost filter, its interval's
-# link + area + error), the executed-instruction count of the stage-1 kernel on config 3 from the ncu capture in
-# profiles/ (2*DFMA + DMUL + DADD thread instructions / boundary points) -- see DESIGN.md "Roofline".
-FLOP_PER_POINT = 2155.0
-# DRAM bytes of one stage-1 launch on config 3 (dram__bytes_read.sum + dram__bytes_write.sum of the same capture,
-# profiles/r01b_ncu_full.csv): 0.10 GB read + 4.05 GB written, of which 4.0 GB is the hand-over arena
-STAGE1_DRAM_BYTES_CONFIG3 = 4.147e9
 FP64_LANES_PER_SM = 64          # FP64 FMA lanes per SM (derivation of the ALU peak)
+COUNTS = os.path.join(ROOT, "profiles", "r02_counts.json")
+# the workloads of the bench: the headline first, then the ones reported under "other_configs"
+OTHER = ["config2", "config4", "config5", "fig5_resonant"]
+NCU_METRICS = ("gpu__time_duration.sum,smsp__sass_thread_inst_executed_op_dfma_pred_on.sum,"
+               "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum,smsp__sass_thread_inst_executed_op_dadd_pred_on.sum,"
+               "dram__bytes_read.sum,dram__bytes_write.sum,sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active,"
+               "smsp__issue_active.avg.pct_of_peak_sustained_active")
+STAGES = ("seeds_kernel", "stage1_kernel", "adaptive_kernel", "adaptive_kernel")      # launch order inside one twk_magnify
 
 
 def parse_args():
@@ -46,10 +60,14 @@ def parse_args():
     ap.add_argument("--workload", default="config3")
     ap.add_argument("--cpu-sample", type=int, default=0, help="sources in the cpu_baseline sample (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true")
+    ap.add_argument("--profile-pass", action="store_true")
+    ap.add_argument("--parse-ncu", default=None)
+    ap.add_argument("--scaling", action="store_true")
     return ap.parse_args()
 
 
-def make_workload(name, rank, **size):
+def make_workload(name, rank=0, **size):
     """The batch of rank `rank`: every rank draws its own seeded batch (independent problems, no collective on the
     data path -- P:392 "no communication between devices")."""
     import workloads as W
@@ -57,6 +75,8 @@ def make_workload(name, rank, **size):
         return W.config3(seed=250103322 + rank, **size)
     if name == "config5":
         return W.config5(seed=250103323 + rank)
+    if name.startswith("fig5_"):
+        return W.fig5_map(name[5:])
     return W.get(name)
 
 
@@ -107,7 +127,8 @@ class ClockSampler:
 
 
 def cpu_baseline(wl, n_sample, tol):
-    """The oracle as it stands (paper-style sampler, double) on a bounded seeded sample of the workload."""
+    """The oracle as it stands (paper-style sampler, double) on a bounded seeded sample of the workload: all host cores,
+    and one core on a tenth of that sample."""
     from oracle import api
     n_sample = min(n_sample, wl.n_sources)
     idx = np.sort(np.random.default_rng(12345).choice(wl.n_sources, n_sample, replace=False))
@@ -116,10 +137,18 @@ def cpu_baseline(wl, n_sample, tol):
     t0 = time.perf_counter()
     r = api.magnify(sub, tol, mode=0, prec=0, nthreads=cores)
     dt = time.perf_counter() - t0
+    n1 = max(200, n_sample // (10 * max(cores // 2, 1)))
+    sub1 = wl.subset(idx[:: max(1, n_sample // n1)][:n1])
+    t0 = time.perf_counter()
+    api.magnify(sub1, tol, mode=0, prec=0, nthreads=1)
+    dt1 = time.perf_counter() - t0
     return {"value": n_sample / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{n_sample} seeded-random sources of {wl.name} (of {wl.n_sources}), oracle paper-style sampler, "
                       f"double, tol {tol:g}, {dt:.1f} s wall, mean {float(r['nsamples'].mean()):.1f} samples/source",
-            "seconds": dt}
+            "seconds": dt,
+            "one_core": {"value": sub1.n_sources / dt1, "unit": UNIT, "cores": 1, "seconds": dt1,
+                         "sample": f"{sub1.n_sources} of those sources on one thread"},
+            "per_core_of_all_cores": n_sample / dt / cores}
 
 
 def max_over_ranks(values, device, world):
@@ -161,10 +190,112 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+# ---------------------------------------------------------------------------------------------------------------------
+# executed-instruction counts from ncu (profiles/r02_counts.json)
+# ---------------------------------------------------------------------------------------------------------------------
+def library_source_hash():
+    import paper_2501_03322_b200 as P
+    v = P.twk_version()
+    return v.split("src:")[1].strip() if "src:" in v else None
+
+
+def parse_ncu(path):
+    """ncu --csv log of `bench.py --profile-pass` -> profiles/r02_counts.json.  The pass launches, for every workload in
+    order, the kernels of one twk_magnify call (STAGES); rows are grouped by launch ID."""
+    launches = {}
+    with open(path, newline="") as f:
+        rows = [r for r in csv.reader(f) if len(r) >= 15 and r[0].isdigit()]
+    for r in rows:
+        lid = int(r[0])
+        d = launches.setdefault(lid, {"kernel": r[4]})
+        try:
+            d[r[12]] = float(r[14].replace(",", ""))
+        except ValueError:
+            pass
+    order = [launches[k] for k in sorted(launches)]
+    names = ["config3"] + OTHER
+    per = len(STAGES)
+    assert len(order) == per * len(names), (len(order), per * len(names))
+    out = {"source_hash": library_source_hash(), "workloads": {},
+           "command": "ncu --metrics " + NCU_METRICS + " --clock-control none --csv --log-file gpurun_out/r02_counts.csv "
+                      "python bench.py --profile-pass ; python bench.py --parse-ncu gpurun_out/r02_counts.csv",
+           "note": "per kernel launch of ONE twk_magnify call: executed thread-level FP64 instructions, flop = 2 dfma + "
+                   "dmul + dadd, DRAM bytes, duration under ncu (serialised, cold cache), FP64-pipe and issue activity"}
+    for w, name in enumerate(names):
+        ks = {}
+        for s, stage in enumerate(STAGES):
+            L = order[w * per + s]
+            assert stage in L["kernel"], (stage, L["kernel"])
+            dfma = L["smsp__sass_thread_inst_executed_op_dfma_pred_on.sum"]
+            dmul = L["smsp__sass_thread_inst_executed_op_dmul_pred_on.sum"]
+            dadd = L["smsp__sass_thread_inst_executed_op_dadd_pred_on.sum"]
+            ks[f"stage{s}"] = {"kernel": stage, "dfma": dfma, "dmul": dmul, "dadd": dadd, "flop": 2 * dfma + dmul + dadd,
+                               "dram_bytes": L["dram__bytes_read.sum"] + L["dram__bytes_write.sum"],
+                               "ncu_ms": L["gpu__time_duration.sum"] * 1e-6,
+                               "fp64_pipe_pct": L["sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active"],
+                               "issue_active_pct": L["smsp__issue_active.avg.pct_of_peak_sustained_active"]}
+        out["workloads"][name] = ks
+    os.makedirs(os.path.dirname(COUNTS), exist_ok=True)
+    with open(COUNTS, "w") as f:
+        json.dump(out, f, indent=1)
+    print("wrote", COUNTS, "source hash", out["source_hash"])
+
+
+def load_counts():
+    try:
+        c = json.load(open(COUNTS))
+    except Exception:
+        return None, "profiles/r02_counts.json missing"
+    h = library_source_hash()
+    if not h or c.get("source_hash") != h:
+        return None, f"profiles/r02_counts.json was measured on sources {c.get('source_hash')}, the library is {h}: stale"
+    return c, None
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def time_workload(P, torch, wl, dev, steps, warmup, barrier, want_e2e=False):
+    """Device-resident timing of `steps` twk_magnify calls on `wl` (after `warmup`), then the per-stage durations from
+    the library's own CUDA events in a separate pass (no synchronisation inside the timed loop)."""
+    n = wl.n_sources
+    ctx = P.Context(n)
+    d = ctx.upload(wl, dev)
+    out = dict(out_mu=torch.empty(n, dtype=torch.float64, device=dev), out_err=torch.empty(n, dtype=torch.float64, device=dev),
+               out_nsamples=torch.empty(n, dtype=torch.int32, device=dev), out_status=torch.empty(n, dtype=torch.int32, device=dev))
+
+    def step():
+        ctx.twk_magnify(d["s"], d["q"], d["rho"], d["zeta"], d["model_id"], wl.rel_tol, **out)
+
+    for _ in range(max(warmup, 3)):
+        step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    ctx.twk_enable_stage_timing(True)
+    stage = []
+    for _ in range(steps):
+        step()
+        stage.append(ctx.twk_last_stage_ms())
+    ctx.twk_enable_stage_timing(False)
+    stats = ctx.twk_last_stats()
+    r = {"ms": ms, "stage_ms": {k: float(np.mean([x[k] for x in stage])) for k in ("stage0", "stage1", "stage2", "stage3")},
+         "n_stage2": stats["n_stage2"], "n_stage3": stats["n_stage3"], "launches": stats["n_launches"],
+         "total_points": int(out["out_nsamples"].to(torch.int64).sum().item()),
+         "converged": int((out["out_status"] & 1).ne(0).sum().item()), "ctx": ctx, "d": d, "out": out}
+    return r
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.parse_ncu:
+        parse_ncu(args.parse_ncu)
         return
     import torch
     import torch.distributed as dist
@@ -178,6 +309,20 @@ def main():
         raise SystemExit("bench.py --impl twk needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+
+    if args.profile_pass:                   # what the ncu counting pass runs: one call per workload, nothing else
+        for name in ["config3"] + OTHER:
+            wl = make_workload(name)
+            ctx = P.Context(wl.n_sources)
+            d = ctx.upload(wl, dev)
+            ctx.twk_magnify(d["s"], d["q"], d["rho"], d["zeta"], d["model_id"], wl.rel_tol)
+            torch.cuda.synchronize()
+            ctx.close()
+        return
+    if args.scaling:
+        run_scaling(P, torch, dev)
+        return
+
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
@@ -188,35 +333,12 @@ def main():
 
     wl = make_workload(args.workload, rank)
     n = wl.n_sources
-    ctx = P.Context(n)
-    ctx.twk_enable_stage_timing(True)
-    d = ctx.upload(wl, dev)
-    out = dict(out_mu=torch.empty(n, dtype=torch.float64, device=dev), out_err=torch.empty(n, dtype=torch.float64, device=dev),
-               out_nsamples=torch.empty(n, dtype=torch.int32, device=dev), out_status=torch.empty(n, dtype=torch.int32, device=dev))
-
-    def step():
-        ctx.twk_magnify(d["s"], d["q"], d["rho"], d["zeta"], d["model_id"], wl.rel_tol, **out)
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
     sampler = ClockSampler(local) if rank == 0 else None
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    stage_ms = []
     barrier()
-    e0.record()
-    for _ in range(args.steps):
-        step()
-        stage_ms.append(ctx.twk_last_stage_ms())      # CUDA events recorded by the library on this stream
-    e1.record()
-    barrier()
-    ms = e0.elapsed_time(e1)
+    R = time_workload(P, torch, wl, dev, args.steps, args.warmup, barrier)
     clocks = sampler.stop() if sampler else None
-    stats = ctx.twk_last_stats()
-    nsamp = out["out_nsamples"].to(torch.int64)
-    total_points = int(nsamp.sum().item())
-    status = out["out_status"]
-    n_conv = int((status & 1).ne(0).sum().item())
+    ctx, d, out = R["ctx"], R["d"], R["out"]
+    ms = R["ms"]
 
     # ---- end to end: pinned host buffers through twk_magnify_host -----------------------------------------------
     hs = {k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in
@@ -256,6 +378,7 @@ def main():
     ps_fraction = float((out_ps["out_status"] & 64).ne(0).double().mean().item())
     ps_maxdev = float(((out_ps["out_mu"] / out["out_mu"]) - 1).abs().max().item())
     ctx_ps.close()
+    ctx.close()
 
     ms, ms_e2e, ms_ps = max_over_ranks([ms, ms_e2e, ms_ps], dev, world)
 
@@ -269,20 +392,36 @@ def main():
         sm_max_mhz = float(peaks.get("sm_max_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0)
         peak_tf = props.multi_processor_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
         probe_tf = P.twk_fp64_peak_probe(1 << 16)
-        s1 = float(np.mean([x["stage1"] for x in stage_ms]))
-        s2 = float(np.mean([x["stage2"] for x in stage_ms]))
-        s3 = float(np.mean([x["stage3"] for x in stage_ms]))
-        flop_launch = FLOP_PER_POINT * 64.0 * n                   # stage 1 solves 64 boundary points per source
-        achieved = flop_launch / (s1 * 1e-3) / 1e12
+        counts, stale = load_counts()
+
+        def fracs(name, stage_ms):
+            """achieved TFLOP/s and fraction of peak per stage, from the ncu counts of this workload and the live times"""
+            if counts is None or name not in counts["workloads"]:
+                return None
+            o = {}
+            for k, c in counts["workloads"][name].items():
+                t = stage_ms.get(k, 0.0)
+                if t > 0 and c["flop"] > 0:
+                    a = c["flop"] / (t * 1e-3) / 1e12
+                    o[k] = {"achieved_tflops": a, "frac": a / peak_tf, "flop": c["flop"], "dram_bytes": c["dram_bytes"],
+                            "fp64_pipe_pct_ncu": c["fp64_pipe_pct"]}
+            return o
+
+        sm = R["stage_ms"]
+        fr = fracs(wl.name, sm) if world == 1 or True else None
+        s1 = sm["stage1"]
+        dom = (fr or {}).get("stage1")
+        step_flop = sum(v["flop"] for v in fr.values()) if fr else None
         line = {
             "metric": METRIC, "value": world * n * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl.name, "sources_per_step_per_gpu": n, "rel_tol": wl.rel_tol, "n_models": wl.n_models,
                        "seed": wl.meta.get("seed"), "parallelism": f"independent batches x{world}, no collective",
-                       "l2": "inputs+outputs per step (~180 MB) exceed the 126 MB L2; no flush needed",
-                       "mean_samples_per_source": total_points / n, "converged_fraction": n_conv / n,
-                       "sources_to_stage2": stats["n_stage2"], "sources_to_stage3": stats["n_stage3"]},
+                       "l2": "inputs+outputs per step (~180 MB) and the per-step workspace traffic (seed blocks 1 GB, "
+                             "hand-over arena 4 GB) exceed the 126 MB L2; no flush needed",
+                       "mean_samples_per_source": R["total_points"] / n, "converged_fraction": R["converged"] / n,
+                       "sources_to_stage2": R["n_stage2"], "sources_to_stage3": R["n_stage3"]},
             "e2e": {"value": world * n * args.steps / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e / args.steps},
             "with_point_source_test": {"value": world * n * args.steps / (ms_ps * 1e-3), "unit": UNIT,
@@ -290,29 +429,81 @@ def main():
                                        "max_rel_dev_from_contour": ps_maxdev,
                                        "note": "option point_source_test=1 (SURVEY N1, P:122): sources passing the "
                                                "quadrupole and ghost-image tests skip the contour; NOT the headline"},
-            "gpu_launches": stats["n_launches"] * args.steps,
+            "gpu_launches": R["launches"] * args.steps,
             "clocks": clocks,
-            "roofline": {"bound": "alu", "kernel": "stage1_kernel (64 point solves + 64 intervals per source)",
-                         "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
-                         "traffic": STAGE1_DRAM_BYTES_CONFIG3 if wl.name == "config3" else None,
-                         "traffic_note": "DRAM bytes per stage-1 launch from profiles/r01b_ncu_full.csv; algorithmic "
-                                         "bytes are 45 B/source = 0.18 GB, the rest is the hand-over arena to stage 2",
+            "roofline": {"bound": "alu", "kernel": "stage1_kernel (64 seeded point solves + 64 intervals per source)",
+                         "achieved": dom["achieved_tflops"] if dom else None, "peak": peak_tf, "unit": "TFLOP/s",
+                         "frac": dom["frac"] if dom else None,
+                         "traffic": dom["dram_bytes"] if dom else None,
+                         "counts": "profiles/r02_counts.json (ncu, executed DFMA/DMUL/DADD per launch, keyed by the source "
+                                   "hash in twk_version())" if dom else stale,
+                         "traffic_note": "DRAM bytes of one stage-1 launch (ncu); algorithmic bytes are 45 B/source = "
+                                         "0.18 GB, the rest is the seed blocks read (1 GB) and the hand-over arena written",
                          "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x "
                                         f"{sm_max_mhz:.0f} MHz (MEASURED_PEAKS.json has no FP64 figure)",
-                         "peak_probe_tflops": probe_tf, "frac_of_probe": achieved / probe_tf,
-                         "flop_per_point": FLOP_PER_POINT, "points_per_launch": 64 * n,
-                         "kernel_ms": {"stage1": s1, "stage2": s2, "stage3": s3},
-                         "stage1_share_of_step": s1 / (ms / args.steps),
-                         "point_solves_per_s": total_points * args.steps / (ms * 1e-3)},
+                         "peak_probe_tflops": probe_tf, "frac_of_probe": (dom["achieved_tflops"] / probe_tf) if dom else None,
+                         "flop_per_point": (dom["flop"] / (64.0 * n)) if dom else None, "points_per_launch": 64 * n,
+                         "kernel_ms": sm, "stage1_share_of_step": s1 / (ms / args.steps),
+                         "per_stage": fr,
+                         "whole_step_frac": (step_flop / (ms / args.steps * 1e-3) / 1e12 / peak_tf) if step_flop else None,
+                         "point_solves_per_s": R["total_points"] * args.steps / (ms * 1e-3)},
         }
+        if world == 1 and not args.no_other_configs:
+            other = {}
+            for name in OTHER:
+                w2 = make_workload(name)
+                r2 = time_workload(P, torch, w2, dev, max(args.steps, 5), 3, barrier)
+                r2["ctx"].close()
+                f2 = fracs(name, r2["stage_ms"])
+                other[name] = {"value": w2.n_sources * max(args.steps, 5) / (r2["ms"] * 1e-3), "unit": UNIT,
+                               "sources": w2.n_sources, "rel_tol": w2.rel_tol, "ms_per_step": r2["ms"] / max(args.steps, 5),
+                               "kernel_ms": r2["stage_ms"], "sources_to_stage2": r2["n_stage2"],
+                               "sources_to_stage3": r2["n_stage3"], "mean_samples_per_source": r2["total_points"] / w2.n_sources,
+                               "converged_fraction": r2["converged"] / w2.n_sources,
+                               "stage2_frac": (f2 or {}).get("stage2", {}).get("frac") if f2 else None,
+                               "per_stage": f2}
+            line["other_configs"] = other
         if world == 1 and not args.no_cpu_baseline:
             from oracle import api as _api
             ns = args.cpu_sample or min(n, 15000 * _api.num_threads())
             line["cpu_baseline"] = cpu_baseline(wl, ns, wl.rel_tol)
         print(json.dumps(line))
-    ctx.close()
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_scaling(P, torch, dev):
+    """Time of one twk_magnify call against the number of sources N_source (Fig.8): evenly spaced subsets of
+    config 3, device-resident, best of 5 after 2 warm-up calls.  Writes profiles/r02_scaling.csv."""
+    full = make_workload("config3")
+    sizes = [1, 8, 64, 148, 296, 592, 888, 1184, 2368, 4736, 9472, 18944, 37888, 56832, 113664, 227328, 500000, 1000000, 2000000,
+             4096000]
+    rows = []
+    for ns in sizes:
+        idx = np.unique(np.linspace(0, full.n_sources - 1, ns).astype(np.int64))
+        wl = full.subset(idx)
+        ctx = P.Context(wl.n_sources)
+        d = ctx.upload(wl, dev)
+        best = 1e30
+        for it in range(7):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.twk_magnify(d["s"], d["q"], d["rho"], d["zeta"], d["model_id"], wl.rel_tol)
+            e1.record()
+            torch.cuda.synchronize()
+            if it >= 2:
+                best = min(best, e0.elapsed_time(e1))
+        st = ctx.twk_last_stats()
+        ctx.close()
+        rows.append((wl.n_sources, best, wl.n_sources / (best * 1e-3), st["n_stage2"], st["n_stage3"]))
+        print(rows[-1], flush=True)
+    path = os.path.join(ROOT, "profiles", "r02_scaling.csv")
+    with open(path, "w") as f:
+        f.write("# python bench.py --scaling   (one B200; evenly spaced subsets of config 3, tol 1e-4, best of 5 calls)\n")
+        f.write("n_sources,ms_per_call,magnifications_per_s,sources_to_stage2,sources_to_stage3\n")
+        for r in rows:
+            f.write("%d,%.5f,%.4e,%d,%d\n" % r)
+    print("wrote", path)
 
 
 if __name__ == "__main__":

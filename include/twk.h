@@ -51,10 +51,11 @@ extern "C" {
 
 typedef struct twk_ctx twk_ctx; /* opaque; owns only its device scratch workspace */
 
+/* Not options of this build: the 64 new boundary samples (= quantiles) per refinement iteration ("the
+ * number is adjustable") and the 64 uniform samples of the first iteration.  One thread solves one new sample and
+ * two warps own one source; every shared-memory tile, scan and compaction of the kernels is laid out for that width, so
+ * it is a compile-time constant (kThreads in csrc/twk_kernels.cuh), not a run-time field. */
 typedef struct {
-  int samples_per_iter; /* new boundary samples (= quantiles) per refinement iteration, default 64;  */
-                        /* must be 64 in this build (one thread per new sample, two warps per source)             */
-  int initial_samples;  /* uniform samples of the first iteration, default 64; must be 64 in this build    */
   int max_samples;      /* sample cap per source, default 4096; 64 <= max_samples <= 4096                  */
   int subtract_avg_tol; /* 1 = subtract the average tolerance from every interval error before sampling */
   int64_t handoff_slots; /* slots of the hand-over arena through which the first iteration (64 records, interval     */
@@ -169,6 +170,14 @@ int twk_last_stage_ms(twk_ctx* ctx, float* ms4);
  * (8 independent chains per thread, a full persistent grid) and returns the measured TFLOP/s (2 flop per DFMA) in
  * *out_tflops.  Synchronous. */
 int twk_fp64_peak_probe(int iters, double* out_tflops);
+
+/* Debug build only (libtwk_debug.so, compiled with -DTWK_DEBUG; twk_version() says so): the kernels count violations of
+ * their own invariants instead of trapping -- out8 = {record id out of range, sample angles not strictly increasing,
+ * sorted list not a permutation of the sample ids, two writers to one record in one re-judging phase, worklist / hand-over
+ * slot out of range, new angle outside its interval, sources checked, iterations checked}.  Synchronises the device;
+ * reset != 0 clears the counters.  Returns TWK_EINVAL in the release build.  Stands in for compute-sanitizer, which this
+ * pool does not offer. */
+int twk_debug_counters(uint32_t* out8, int reset);
 
 const char* twk_strerror(int code);
 const char* twk_version(void);

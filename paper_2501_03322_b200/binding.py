@@ -11,14 +11,15 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(HERE, "libtwk.so")
+# TWK_LIBRARY selects another build of the same sources (the -DTWK_DEBUG build libtwk_debug.so of tests/test_gpu_debug.py)
+_LIB_PATH = os.environ.get("TWK_LIBRARY") or os.path.join(HERE, "libtwk.so")
 _lib = None
 
 TWK_ST_CONVERGED, TWK_ST_CAP, TWK_ST_REPAIRED, TWK_ST_DOMAIN, TWK_ST_NUMERIC, TWK_ST_SLOPE, TWK_ST_POINT = 1, 2, 4, 8, 16, 32, 64
 
 SYMBOLS = ["twk_default_options", "twk_create", "twk_destroy", "twk_workspace_bytes", "twk_magnify", "twk_magnify_lightcurve",
            "twk_images_fixed", "twk_images_fixed_seeded", "twk_stage1_records",
-           "twk_magnify_host", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_strerror", "twk_version"]
+           "twk_magnify_host", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_debug_counters", "twk_strerror", "twk_version"]
 
 
 class TwkError(RuntimeError):
@@ -26,7 +27,7 @@ class TwkError(RuntimeError):
 
 
 class twk_options(C.Structure):
-    _fields_ = [("samples_per_iter", C.c_int), ("initial_samples", C.c_int), ("max_samples", C.c_int),
+    _fields_ = [("max_samples", C.c_int),
                 ("subtract_avg_tol", C.c_int), ("handoff_slots", C.c_int64), ("slope_gate", C.c_double), ("slope_cos", C.c_double), ("point_source_test", C.c_int), ("frame", C.c_int)]
 
 
@@ -59,6 +60,7 @@ def lib():
         L.twk_enable_stage_timing.argtypes = [vp, i32]
         L.twk_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.twk_fp64_peak_probe.argtypes = [i32, C.POINTER(dbl)]
+        L.twk_debug_counters.argtypes = [C.POINTER(C.c_uint32), i32]
         L.twk_strerror.argtypes = [i32]
         L.twk_strerror.restype = C.c_char_p
         L.twk_version.restype = C.c_char_p
@@ -93,6 +95,13 @@ def twk_workspace_bytes(max_sources: int, **opts) -> int:
 
 def twk_version() -> str:
     return lib().twk_version().decode()
+
+
+def twk_debug_counters(reset: bool = False):
+    """Invariant-violation counters of the debug build (raises TwkError on the release build)."""
+    out = (C.c_uint32 * 8)()
+    _check(lib().twk_debug_counters(out, 1 if reset else 0), "twk_debug_counters")
+    return [int(x) for x in out]
 
 
 def twk_fp64_peak_probe(iters: int = 1 << 16) -> float:

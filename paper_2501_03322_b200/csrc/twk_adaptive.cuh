@@ -67,6 +67,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   // record of sample id: ids 0..63 of a handed-over source live in its hand-over slot ([26][64]), the rest in the arena
   const double* hand = nullptr;
   auto recref = [&](int id) -> RecRef {
+    TWK_CHECK(id >= 0 && id < cap, 0);
     if (hand && id < kThreads) return RecRef{const_cast<double*>(hand) + id, kThreads};
     return RecRef{arena + (size_t)id * kRecDoubles, 1};
   };
@@ -79,6 +80,8 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
     const long long cur = iscr[0];
     if (cur >= total) break;
     const long long src = p.list ? (long long)p.list[cur] : cur;
+    TWK_CHECK(src >= 0 && src < p.b.n_sources, 4);
+    if (t == 0) TWK_DEBUG_COUNT(6);
     const SourceParams S = load_source(p.b, src);
     if (!S.valid) {
       if (t == 0) {
@@ -206,6 +209,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
               own = i;
             }
           }
+          TWK_CHECK(own < 0 || th != th || (th > theta[own] && th < ((own + 1 < n) ? theta[own + 1] : kTwoPi)), 5);
           newth[t] = th;
           newint[t] = own;
         }
@@ -266,6 +270,25 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
       }
       const int n_new = n + m;
       __syncthreads();
+#ifdef TWK_DEBUG
+      {   // the sorted list after the merge: angles strictly increasing, ids a permutation of 0 .. n_new - 1
+        unsigned* bits = g_twk_stamp + (size_t)blockIdx.x * 128;
+        for (int i = t; i < 128; i += kThreads) bits[i] = 0u;
+        __syncthreads();
+        for (int i = t; i < n_new; i += kThreads) {
+          TWK_CHECK(i == 0 || theta[i] > theta[i - 1], 1);
+          TWK_CHECK(theta[i] >= 0.0 && theta[i] < kTwoPi, 1);
+          const unsigned id = ids[i];
+          TWK_CHECK(id < (unsigned)n_new, 2);
+          if (id < (unsigned)n_new) {
+            const unsigned old = atomicOr(&bits[id >> 5], 1u << (id & 31));
+            TWK_CHECK(!(old >> (id & 31) & 1u), 2);
+          }
+        }
+        if (t == 0) TWK_DEBUG_COUNT(7);
+        __syncthreads();
+      }
+#endif
       // ---- re-evaluate only the intervals that changed: the one to the left of every new sample, and the
       //      one to its right when the next sample is old (or the list wraps around) ---------------------------------
       int viol = 0;
@@ -311,13 +334,29 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
           __syncthreads();
           const int nv = min(iscr[3], kThreads);
           if (nv == 0) break;
+#ifdef TWK_DEBUG
+          unsigned* bits = g_twk_stamp + (size_t)blockIdx.x * 128;     // one writer per record per phase
+          for (int i = t; i < 128; i += kThreads) bits[i] = 0u;
+          __syncthreads();
+#endif
           if (t < nv && (cint[t] & 256)) {
             const int ib = (newint[t] + 1 < n) ? newint[t] + 1 : 0;
+#ifdef TWK_DEBUG
+            TWK_CHECK(!(atomicOr(&bits[ids[ib] >> 5], 1u << (ids[ib] & 31)) >> (ids[ib] & 31) & 1u), 3);
+#endif
             demote_pair(recref(ids[ib]), cint[t] & 15, (cint[t] >> 4) & 15);
           }
           __syncthreads();
+#ifdef TWK_DEBUG
+          for (int i = t; i < 128; i += kThreads) bits[i] = 0u;
+          __syncthreads();
+#endif
           if (t < nv && !(cint[t] & 256)) {
             const RecRef S5 = recref(ids[newint[t]]);
+#ifdef TWK_DEBUG
+            const unsigned idw = ids[newint[t]];
+            TWK_CHECK(!(atomicOr(&bits[idw >> 5], 1u << (idw & 31)) >> (idw & 31) & 1u), 3);
+#endif
             if (S5.nreal() == 5) demote_pair(S5, cint[t] & 15, (cint[t] >> 4) & 15);
           }
           __syncthreads();
@@ -331,7 +370,9 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
     const int slp = __syncthreads_or(flags & kPointSlope);
     if (t == 0) {
       if (exhausted && !p.final_stage) {
-        p.next_list[atomicAdd(p.next_count, 1)] = (int32_t)src;
+        const int slot = atomicAdd(p.next_count, 1);
+        TWK_CHECK(slot >= 0 && slot < p.b.n_sources, 4);
+        p.next_list[slot] = (int32_t)src;
       } else {
         if (exhausted) status |= 2u;
         if (rep) status |= 4u;

@@ -66,7 +66,7 @@ Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
 }
 
 bool valid_options(const twk_options& o) {
-  return o.samples_per_iter == twk::kThreads && o.initial_samples == twk::kThreads && o.max_samples >= twk::kThreads &&
+  return o.max_samples >= twk::kThreads &&
          o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1) && o.handoff_slots >= -1 && o.slope_gate >= 0.0 && o.slope_cos >= 0.0 && o.slope_cos <= 1.0 &&
          (o.point_source_test == 0 || o.point_source_test == 1) && (o.frame == 0 || o.frame == 1);
 }
@@ -119,8 +119,6 @@ extern "C" {
 
 void twk_default_options(twk_options* opt) {
   if (!opt) return;
-  opt->samples_per_iter = 64;
-  opt->initial_samples = 64;
   opt->max_samples = 4096;
   opt->subtract_avg_tol = 1;
   opt->handoff_slots = -1;
@@ -135,7 +133,15 @@ size_t twk_workspace_bytes(const twk_options* opt, size_t max_sources) {
   twk_default_options(&o);
   if (opt) o = *opt;
   if (!valid_options(o)) return 0;
-  return make_layout(o, max_sources, kAssumedSMs).total;
+  // the refinement stages' record arena scales with the SM count: the current device's when there is one (what
+  // twk_create will allocate), a B200's 148 otherwise (host-side arithmetic, no GPU needed)
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      sms <= 0) {
+    cudaGetLastError();
+    sms = kAssumedSMs;
+  }
+  return make_layout(o, max_sources, sms).total;
 }
 
 int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
@@ -412,15 +418,25 @@ int twk_magnify_host(twk_ctx* ctx, size_t n_models, const double* s, const doubl
   const size_t need = align256(n_models * 8) * 3 + align256(n_sources * 4) + align256(n_sources * 16) +
                       align256(n_sources * 8) * 2 + align256(n_sources * 4) * 2;
   if (need > ctx->stage_bytes) {
+    // (re)allocation happens on the first call and when a batch outgrows the staging area, which then at least doubles:
+    // a sequence of calls of any sizes allocates O(log) times, none in the steady state
     if (ctx->stage) cudaFree(ctx->stage);
     ctx->stage = nullptr;
+    const size_t grown = 2 * ctx->stage_bytes;
     ctx->stage_bytes = 0;
-    cudaError_t e = cudaMalloc((void**)&ctx->stage, need);
+    const size_t want = need > grown ? need : grown;
+    cudaError_t e = cudaMalloc((void**)&ctx->stage, want);
+    if (e != cudaSuccess && want > need) {
+      cudaGetLastError();
+      e = cudaMalloc((void**)&ctx->stage, need);
+      if (e == cudaSuccess) ctx->stage_bytes = need;
+    } else if (e == cudaSuccess) {
+      ctx->stage_bytes = want;
+    }
     if (e != cudaSuccess) {
       cudaGetLastError();
       return e == cudaErrorMemoryAllocation ? TWK_ENOMEM : cuda_fail(e);
     }
-    ctx->stage_bytes = need;
   }
   char* p = ctx->stage;
   double* d_s = (double*)p;      p += align256(n_models * 8);
@@ -484,29 +500,55 @@ int twk_fp64_peak_probe(int iters, double* out_tflops) {
   TWK_CUDA(cudaGetDevice(&dev));
   TWK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   double* d = nullptr;
-  TWK_CUDA(cudaMalloc((void**)&d, 8));
-  cudaEvent_t e0, e1;
-  TWK_CUDA(cudaEventCreate(&e0));
-  TWK_CUDA(cudaEventCreate(&e1));
-  const int grid = sms * 8, block = 256;
-  twk::dfma_probe_kernel<<<grid, block>>>(iters / 8 + 1, d);   // warm-up
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  cudaStream_t st = nullptr;
   float best = 1e30f;
-  for (int rep = 0; rep < 3; ++rep) {
-    TWK_CUDA(cudaEventRecord(e0));
-    twk::dfma_probe_kernel<<<grid, block>>>(iters, d);
-    TWK_CUDA(cudaEventRecord(e1));
-    TWK_CUDA(cudaEventSynchronize(e1));
-    float ms = 0;
-    TWK_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-    if (ms < best) best = ms;
+  const int grid = sms * 8, block = 256;
+  cudaError_t err = cudaMalloc((void**)&d, 8);
+  if (err == cudaSuccess) err = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+  if (err == cudaSuccess) err = cudaEventCreate(&e0);
+  if (err == cudaSuccess) err = cudaEventCreate(&e1);
+  if (err == cudaSuccess) {
+    twk::dfma_probe_kernel<<<grid, block, 0, st>>>(iters / 8 + 1, d);   // warm-up
+    for (int rep = 0; rep < 3 && err == cudaSuccess; ++rep) {
+      cudaEventRecord(e0, st);
+      twk::dfma_probe_kernel<<<grid, block, 0, st>>>(iters, d);
+      cudaEventRecord(e1, st);
+      err = cudaEventSynchronize(e1);
+      float ms = 0;
+      if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+      if (err == cudaSuccess && ms < best) best = ms;
+    }
+    if (err == cudaSuccess) err = cudaGetLastError();
   }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(d);
-  TWK_CUDA(cudaGetLastError());
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  if (st) cudaStreamDestroy(st);
+  if (d) cudaFree(d);
+  if (err != cudaSuccess) {
+    cudaGetLastError();
+    return cuda_fail(err);
+  }
   const double flop = 2.0 * 8.0 * (double)iters * (double)grid * (double)block;
   *out_tflops = flop / ((double)best * 1e-3) / 1e12;
   return TWK_OK;
+}
+
+int twk_debug_counters(uint32_t* out8, int reset) {
+#ifdef TWK_DEBUG
+  if (!out8) return TWK_EINVAL;
+  TWK_CUDA(cudaDeviceSynchronize());
+  TWK_CUDA(cudaMemcpyFromSymbol(out8, twk::g_twk_debug, 8 * sizeof(uint32_t)));
+  if (reset) {
+    uint32_t z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    TWK_CUDA(cudaMemcpyToSymbol(twk::g_twk_debug, z, sizeof(z)));
+  }
+  return TWK_OK;
+#else
+  (void)out8;
+  (void)reset;
+  return TWK_EINVAL;   // not a debug build
+#endif
 }
 
 const char* twk_strerror(int code) {
@@ -519,6 +561,13 @@ const char* twk_strerror(int code) {
   }
 }
 
-const char* twk_version(void) { return "twk 0.1 (sm_100a)"; }
+#ifndef TWK_SOURCE_HASH
+#define TWK_SOURCE_HASH "unknown"
+#endif
+#ifdef TWK_DEBUG
+const char* twk_version(void) { return "twk 0.2 (sm_100a, TWK_DEBUG) src:" TWK_SOURCE_HASH; }
+#else
+const char* twk_version(void) { return "twk 0.2 (sm_100a) src:" TWK_SOURCE_HASH; }
+#endif
 
 }  // extern "C"

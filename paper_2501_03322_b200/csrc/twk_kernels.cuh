@@ -17,6 +17,32 @@
 
 namespace twk {
 
+// ------------------------------------------------------------------------------------------------------------
+// Debug build (-DTWK_DEBUG, libtwk_debug.so): the builder's own invariants, counted instead of trapped so that a
+// violated one does not take the context down.  compute-sanitizer is not available on this pool; these checks are what
+// stands in for memcheck / racecheck on the data-dependent indexing of the refinement kernels (tests/test_gpu_debug.py).
+//   [0] record id outside the CTA's arena            [1] sample angles not strictly increasing after an iteration
+//   [2] sorted list is not a permutation of the ids  [3] a record re-judged by two threads in one phase
+//   [4] worklist / hand-over slot out of range       [5] a new angle outside the interval that owns its quantile
+//   [6] sources checked by the refinement stages     [7] iterations checked
+// ------------------------------------------------------------------------------------------------------------
+#ifdef TWK_DEBUG
+__device__ unsigned g_twk_debug[8];
+__device__ unsigned g_twk_stamp[2048 * 64];   // one bit per record of every CTA's arena slot (<= 2048 CTAs x 4096 records)
+#define TWK_CHECK(cond, which)                            \
+  do {                                                    \
+    if (!(cond)) atomicAdd(&twk::g_twk_debug[which], 1u); \
+  } while (0)
+#define TWK_DEBUG_COUNT(which) atomicAdd(&twk::g_twk_debug[which], 1u)
+#else
+#define TWK_CHECK(cond, which) \
+  do {                         \
+  } while (0)
+#define TWK_DEBUG_COUNT(which) \
+  do {                         \
+  } while (0)
+#endif
+
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr double kPi = 3.141592653589793238462643383279;
 constexpr double kInvPi = 0.318309886183790671537767526745;

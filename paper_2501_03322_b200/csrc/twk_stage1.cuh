@@ -213,6 +213,7 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
         // a9: append to the refinement worklist; hand the first-iteration state over when a slot is free
         if (t == 0) {
           const int slot = atomicAdd(p.list_count, 1);
+          TWK_CHECK(slot >= 0 && slot < n, 4);
           p.list[slot] = (int32_t)(base + i);
           iscr[3] = slot;
         }
