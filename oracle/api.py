@@ -28,7 +28,7 @@ def lib():
         L.orc_images_fixed.argtypes = [C.c_int64, _D, _D, _D, C.c_int64, _I32, _D, C.c_int, C.c_int, C.c_int,
                                        _D, _I8, _I8, _D, _D, _I32, _D]
         L.orc_magnify.argtypes = [C.c_int64, _D, _D, _D, C.c_int64, _I32, _D, C.c_double, C.c_int, C.c_int, C.c_int,
-                                  C.c_int, C.c_int, C.c_int, C.c_int, _D, _D, _I32, _U32, C.c_double, C.c_double]
+                                  C.c_int, C.c_int, C.c_int, C.c_int, _D, _D, _I32, _U32, C.c_double, C.c_double, C.c_int]
         L.orc_point_source.argtypes = [C.c_int64, _D, _D, _D, C.c_int64, _I32, _D, C.c_double, C.c_int, _I8, _D, _D, _D]
         L.orc_magnify_thetas.argtypes = [C.c_double] * 6 + [C.c_int] * 5 + [_D]
         L.orc_magnify_thetas.restype = C.c_int
@@ -110,9 +110,10 @@ def images_fixed(wl, N=None, prec=0, nthreads=0, want_z=True, want_piece=False):
 
 
 def magnify(wl, rel_tol=None, mode=0, prec=0, nthreads=0, samples_per_iter=64, initial_samples=64, max_samples=4096,
-            subtract_avg_tol=1, slope_gate=1e-5, slope_cos=0.70710678118654752):
+            subtract_avg_tol=1, slope_gate=1e-5, slope_cos=0.70710678118654752, hidden_guard=0):
     """Adaptive face over a Workload.  mode 0 = the paper's sampler, mode 1 = converged reference (bisection).
-    slope_gate: proximity gate of the slope detector (0 = off).  Returns dict(mu, err, nsamples, status)."""
+    slope_gate: proximity gate of the slope detector (0 = off).  hidden_guard=1 adds the L-4 hidden-crossing
+    term to the interval estimates (an extension).  Returns dict(mu, err, nsamples, status)."""
     s, q, rho, mid, zeta = _batch(wl)
     n = zeta.shape[0]
     tol = float(wl.rel_tol if rel_tol is None else rel_tol)
@@ -121,7 +122,7 @@ def magnify(wl, rel_tol=None, mode=0, prec=0, nthreads=0, samples_per_iter=64, i
     st = np.zeros(n, np.uint32)
     lib().orc_magnify(len(s), _p(s, _D), _p(q, _D), _p(rho, _D), n, _p(mid, _I32), _p(zeta, _D), tol, mode, samples_per_iter,
                       initial_samples, max_samples, subtract_avg_tol, prec, nthreads, _p(mu, _D), _p(err, _D), _p(ns, _I32),
-                      _p(st, _U32), float(slope_gate), float(slope_cos))
+                      _p(st, _U32), float(slope_gate), float(slope_cos), int(hidden_guard))
     return dict(mu=mu, err=err, nsamples=ns, status=st)
 
 

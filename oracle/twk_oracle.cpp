@@ -245,6 +245,9 @@ void point_solve(const Lens<R>& L, const Cx<R>& zc, R rho, R theta, Sample<R>& S
   }
 }
 
+const double kPi = 3.14159265358979323846264338327950288;
+template <class R> R pi_v() { return std::acos(R(-1)); }
+
 // ---------------------------------------------------------------------------------------------------------
 // O6 + O7: one interval (theta_i -> theta_{i+1}): link, area piece, error piece.
 // ---------------------------------------------------------------------------------------------------------
@@ -377,8 +380,57 @@ void eval_interval(const Sample<R>& A, const Sample<R>& B, R dth, Piece<R>& P, R
   P.terms[4] = E1; P.terms[5] = E2; P.terms[6] = E3; P.terms[7] = dAp;
 }
 
-const double kPi = 3.14159265358979323846264338327950288;
-template <class R> R pi_v() { return std::acos(R(-1)); }
+
+// ---------------------------------------------------------------------------------------------------------
+// L-4 guard (an EXTENSION of the paper's estimate, off by default; reading L-4).  The estimates of Eq.(17)
+// see an interval through its end points only: a boundary that dips into a caustic and out again BETWEEN two adjacent
+// samples (both with 3 images) leaves no trace in them.  The ghost pair does: next to a fold its separation squared
+// D = |z_a - z_b|^2 is proportional to the distance of the boundary point from the caustic, so along the boundary it
+// follows a parabola in theta that reaches zero where the boundary touches the caustic and would turn negative inside,
+// where the pair is real with the same separation law.  For the interval (A, B), D is fitted through (A-, A, B) and
+// through (A, B, B+) (neighbours with 3 images only); a convex fit whose vertex lies inside the interval at a negative
+// value D* means a hidden pair of crossings 2 sqrt(-D*/C) apart (C = the fit's curvature), whose images enclose the
+// area  v (pi/2) (-D*) / sqrt(C)  (half an ellipse: pair separation sqrt(-D) across, v = speed of the pair's midpoint
+// along the critical curve, taken from the ghost midpoints of A and B).  That area is added to the interval's error
+// estimate, so the sampler refines there until the crossings are seen or the hidden area is negligible.
+// dm, d, dp = theta_A - theta_A-, theta_B - theta_A, theta_B+ - theta_B  (> 0).
+// ---------------------------------------------------------------------------------------------------------
+template <class R>
+bool ghost_pair(const Sample<R>& S, Cx<R>& sep, Cx<R>& mid) {
+  if (S.nreal != 3) return false;
+  int g[2], ng = 0;
+  for (int k = 0; k < 5 && ng < 2; ++k)
+    if (S.kind[k] == 0) g[ng++] = k;
+  if (ng != 2) return false;
+  sep = S.z[g[0]] - S.z[g[1]];
+  mid = R(0.5) * (S.z[g[0]] + S.z[g[1]]);
+  return true;
+}
+
+template <class R>
+R hidden_crossing_term(const Sample<R>* Am, const Sample<R>& A, const Sample<R>& B, const Sample<R>* Bp, R dm, R d, R dp) {
+  Cx<R> sA, mA, sB, mB, s3, m3;
+  if (!ghost_pair(A, sA, mA) || !ghost_pair(B, sB, mB)) return R(0);
+  const R DA = std::norm(sA), DB = std::norm(sB);
+  const R v = std::abs(mB - mA) / d;
+  R term = 0;
+  for (int side = 0; side < 2; ++side) {
+    const Sample<R>* T = side ? Bp : Am;
+    if (!T || !ghost_pair(*T, s3, m3)) continue;
+    // three points (x0,y0),(x1,y1),(x2,y2) in theta - theta_A, in increasing order
+    const R x0 = side ? R(0) : -dm, x1 = side ? d : R(0), x2 = side ? d + dp : d;
+    const R y0 = side ? DA : std::norm(s3), y1 = side ? DB : DA, y2 = side ? std::norm(s3) : DB;
+    const R f01 = (y1 - y0) / (x1 - x0), f12 = (y2 - y1) / (x2 - x1);
+    const R C = (f12 - f01) / (x2 - x0);
+    if (!(C > 0)) continue;
+    const R xs = R(0.5) * (x0 + x1) - f01 / (R(2) * C);
+    if (!(xs > 0 && xs < d)) continue;
+    const R ys = y0 + f01 * (xs - x0) + C * (xs - x0) * (xs - x1);
+    if (!(ys < 0)) continue;
+    term = std::max(term, v * R(0.5) * pi_v<R>() * (-ys) / std::sqrt(C));
+  }
+  return term;
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // Fixed-sampling face: theta_j = 2 pi j / N.
@@ -429,6 +481,7 @@ struct AdaptOpt {
   int samples_per_iter, initial_samples, max_samples, subtract_avg_tol;
   double slope_gate;   // slope detector proximity gate (0 = off)
   double slope_cos;    // largest |cos| still counted as perpendicular (cos 45 deg: reading G-4)
+  int hidden_guard;    // L-4 guard (extension, default 0)
 };
 
 template <class R> struct Contour {
@@ -440,6 +493,7 @@ template <class R> struct Contour {
   R twopi;
   R gate2 = R(0);             // square of the slope detector's gate
   R cos2 = R(0.5);            // square of the largest |cos| counted as perpendicular
+  int guard = 0;              // L-4 guard: add the hidden-crossing term to the interval estimates
   void init(int n0) {
     S.resize(n0);
     for (int j = 0; j < n0; ++j) point_solve(L, zc, rho, twopi * R(j) / R(n0), S[j]);
@@ -480,6 +534,10 @@ template <class R> struct Contour {
   void eval(int i) {
     const int n = (int)S.size();
     eval_interval(S[i], S[(i + 1) % n], dtheta(i), P[i], gate2, cos2);
+    if (guard && n >= 4 && !P[i].bad && P[i].crossing == 0) {
+      const int im = (i + n - 1) % n, ib = (i + 1) % n, ip = (i + 2) % n;
+      P[i].err += hidden_crossing_term(&S[im], S[i], S[ib], &S[ip], dtheta(im), dtheta(i), dtheta(ib));
+    }
   }
   // insert new angles (each strictly inside some interval), re-evaluate only the changed intervals
   void insert(std::vector<R> th) {
@@ -589,6 +647,7 @@ void magnify_one(double s, double q, double rho_, double zre, double zim, double
   C.twopi = R(2) * pi_v<R>();
   C.gate2 = R(o.slope_gate) * R(o.slope_gate);
   C.cos2 = R(o.slope_cos) * R(o.slope_cos);
+  C.guard = o.hidden_guard;
   const R rtol = (R)tol;
   uint32_t status = 0;
   if (!(s > 0) || !(q > 0) || !(rho_ > 0) || !std::isfinite(s) || !std::isfinite(q) || !std::isfinite(rho_) ||
@@ -837,8 +896,9 @@ void orc_images_fixed(int64_t n_models, const double* s, const double* q, const 
 void orc_magnify(int64_t n_models, const double* s, const double* q, const double* rho, int64_t n_sources,
                  const int32_t* model_id, const double* zeta, double rel_tol, int mode, int samples_per_iter,
                  int initial_samples, int max_samples, int subtract_avg_tol, int prec, int nthreads, double* out_mu,
-                 double* out_err, int32_t* out_nsamples, uint32_t* out_status, double slope_gate, double slope_cos) {
-  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol, slope_gate, slope_cos};
+                 double* out_err, int32_t* out_nsamples, uint32_t* out_status, double slope_gate, double slope_cos,
+                 int hidden_guard) {
+  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol, slope_gate, slope_cos, hidden_guard};
   (void)nthreads;
 #pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads > 0 ? nthreads : orc_num_threads())
   for (int64_t i = 0; i < n_sources; ++i) {
@@ -881,7 +941,7 @@ void orc_point_source(int64_t n_models, const double* s, const double* q, const 
 // Sorted sample angles the paper-style sampler ends with, for one source (diagnostics).  Returns n.
 int orc_magnify_thetas(double s, double q, double rho, double zre, double zim, double rel_tol, int samples_per_iter,
                        int initial_samples, int max_samples, int subtract_avg_tol, int prec, double* out_theta) {
-  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol, 1e-5, 0.70710678118654752};
+  AdaptOpt o{samples_per_iter, initial_samples, max_samples, subtract_avg_tol, 1e-5, 0.70710678118654752, 0};
   int32_t n = 0;
   if (prec) magnify_one<long double>(s, q, rho, zre, zim, rel_tol, 0, o, nullptr, nullptr, &n, nullptr, out_theta);
   else magnify_one<double>(s, q, rho, zre, zim, rel_tol, 0, o, nullptr, nullptr, &n, nullptr, out_theta);

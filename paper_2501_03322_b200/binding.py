@@ -28,7 +28,7 @@ class TwkError(RuntimeError):
 
 class twk_options(C.Structure):
     _fields_ = [("max_samples", C.c_int),
-                ("subtract_avg_tol", C.c_int), ("handoff_slots", C.c_int64), ("slope_gate", C.c_double), ("slope_cos", C.c_double), ("point_source_test", C.c_int), ("frame", C.c_int)]
+                ("subtract_avg_tol", C.c_int), ("handoff_slots", C.c_int64), ("slope_gate", C.c_double), ("slope_cos", C.c_double), ("point_source_test", C.c_int), ("hidden_crossing_guard", C.c_int), ("frame", C.c_int)]
 
 
 def library_path() -> str:

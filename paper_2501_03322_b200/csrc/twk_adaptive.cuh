@@ -22,6 +22,7 @@ struct AdaptArgs {
   double slope_cos2;     // square of the largest |cos| still counted as perpendicular (twk_options.slope_cos)
   int cap;               // sample capacity of this stage (<= 4096)
   int subtract_avg_tol;
+  int guard;             // L-4 guard: hidden-crossing term in the interval estimates (twk_options.hidden_crossing_guard)
   int final_stage;       // 1: cap reached -> return value + estimate with TWK_ST_CAP; 0: hand to next stage
   const int32_t* list;   // worklist of source ids (null: all sources 0..n_sources-1)
   const int* count;      // number of entries of `list` (device; null: n_sources)
@@ -46,6 +47,7 @@ __host__ __device__ inline size_t adaptive_smem_bytes(int cap) {
 
 // 6 CTAs per SM (168 registers): measured 4 / 5 / 6 / 8 CTAs per SM on configs 3 and 5: 9.4 / 9.3 / 8.6 / 8.8 ms and
 // 7.6 / 7.4 / 6.7 / 7.0 ms -- the kernel is latency-bound and wants warps, but at 128 registers it spills
+template <bool kGuard>   // the L-4 hidden-crossing term lives in its own instance of the kernel (see stage1_kernel)
 __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   extern __shared__ double sm[];
   const int cap = p.cap;
@@ -70,6 +72,14 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
     TWK_CHECK(id >= 0 && id < cap, 0);
     if (hand && id < kThreads) return RecRef{const_cast<double*>(hand) + id, kThreads};
     return RecRef{arena + (size_t)id * kRecDoubles, 1};
+  };
+  // L-4 guard term of interval (i, i + 1) in a sorted list of nn samples (neighbours i - 1 and i + 2, cyclic)
+  auto guard_term = [&](int i, int nn) -> double {
+    const int im = (i > 0) ? i - 1 : nn - 1, ib = (i + 1 < nn) ? i + 1 : 0, ip = (ib + 1 < nn) ? ib + 1 : 0;
+    const double dm = (i > 0) ? theta[i] - theta[im] : kTwoPi - theta[im] + theta[i];
+    const double d = (i + 1 < nn) ? theta[ib] - theta[i] : kTwoPi - theta[i] + theta[ib];
+    const double dp = (ib + 1 < nn) ? theta[ip] - theta[ib] : kTwoPi - theta[ib] + theta[ip];
+    return hidden_crossing_term(recref(ids[im]), recref(ids[i]), recref(ids[ib]), recref(ids[ip]), dm, d, dp);
   };
   const long long total = p.count ? (long long)*p.count : p.b.n_sources;
 
@@ -300,7 +310,8 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
           const int ia = pos - 1 + side;                       // interval (ia, ia + 1)
           const int ib = (ia + 1 < n_new) ? ia + 1 : 0;
           const double dth = (ia + 1 < n_new) ? theta[ia + 1] - theta[ia] : kTwoPi - theta[ia];
-          const Piece P = eval_interval(recref(ids[ia]), recref(ids[ib]), dth, p.slope_gate2, p.slope_cos2);
+          Piece P = eval_interval(recref(ids[ia]), recref(ids[ib]), dth, p.slope_gate2, p.slope_cos2);
+          if (kGuard && P.crossing == 0 && n_new >= 4) P.err += guard_term(ia, n_new);
           dA[ia] = P.dA;
           er[ia] = P.err;
           viol |= P.slope;
@@ -320,7 +331,8 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
           for (int i = t; i < n; i += kThreads) {
             const int ib = (i + 1 < n) ? i + 1 : 0;
             const double dth = (i + 1 < n) ? theta[i + 1] - theta[i] : kTwoPi - theta[i];
-            const Piece P = eval_interval_cold(recref(ids[i]), recref(ids[ib]), dth, p.slope_gate2, p.slope_cos2);
+            Piece P = eval_interval_cold(recref(ids[i]), recref(ids[ib]), dth, p.slope_gate2, p.slope_cos2);
+            if (kGuard && P.crossing == 0 && n >= 4) P.err += guard_term(i, n);
             dA[i] = P.dA;
             er[i] = P.err;
             if (P.slope) {

@@ -68,7 +68,8 @@ Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
 bool valid_options(const twk_options& o) {
   return o.max_samples >= twk::kThreads &&
          o.max_samples <= 4096 && (o.subtract_avg_tol == 0 || o.subtract_avg_tol == 1) && o.handoff_slots >= -1 && o.slope_gate >= 0.0 && o.slope_cos >= 0.0 && o.slope_cos <= 1.0 &&
-         (o.point_source_test == 0 || o.point_source_test == 1) && (o.frame == 0 || o.frame == 1);
+         (o.point_source_test == 0 || o.point_source_test == 1) && (o.hidden_crossing_guard == 0 || o.hidden_crossing_guard == 1) &&
+         (o.frame == 0 || o.frame == 1);
 }
 
 int cuda_fail(cudaError_t e) {
@@ -96,7 +97,8 @@ void launch_stage1(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t
   a.group = (int)group;
   const long long groups = (n_sources + group - 1) / group;
   const int grid = (int)(groups < resident ? groups : resident);
-  twk::stage1_kernel<<<grid, twk::kThreads, smem, stream>>>(a);
+  if (a.guard) twk::stage1_kernel<true><<<grid, twk::kThreads, smem, stream>>>(a);
+  else twk::stage1_kernel<false><<<grid, twk::kThreads, smem, stream>>>(a);
 }
 
 struct twk_ctx {
@@ -125,6 +127,7 @@ void twk_default_options(twk_options* opt) {
   opt->slope_gate = 1e-5;
   opt->slope_cos = 0.70710678118654752;
   opt->point_source_test = 0;
+  opt->hidden_crossing_guard = 0;
   opt->frame = 0;
 }
 
@@ -176,8 +179,11 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   }
   // opt in to the large dynamic shared memory of stage 3 (a per-function attribute shared by all contexts, so
   // always the maximum the build supports)
-  e = cudaFuncSetAttribute(twk::adaptive_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  e = cudaFuncSetAttribute(twk::adaptive_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)twk::adaptive_smem_bytes(4096));
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(twk::adaptive_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)twk::adaptive_smem_bytes(4096));
   if (e != cudaSuccess) {
     cudaFree(c->ws);
     delete c;
@@ -249,6 +255,7 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
   a.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
   a.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
   a.subtract_avg_tol = ctx->opt.subtract_avg_tol;
+  a.guard = ctx->opt.hidden_crossing_guard;
   a.out_mu = out_mu;
   a.out_err = out_err;
   a.out_nsamples = out_nsamples;
@@ -279,6 +286,7 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a1.b = a.b;
     a1.tol = rel_tol;
     a1.ps_test = ctx->opt.point_source_test;
+    a1.guard = ctx->opt.hidden_crossing_guard;
     a1.slope_gate2 = ctx->opt.slope_gate * ctx->opt.slope_gate;
     a1.slope_cos2 = ctx->opt.slope_cos * ctx->opt.slope_cos;
     a1.final_stage = P.cap2 ? 0 : 1;
@@ -308,7 +316,8 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a2.next_count = counters + 3;
     a2.handoff = handoff;
     a2.handoff_slots = (long long)ctx->lay.slots;
-    twk::adaptive_kernel<<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2), stream>>>(a2);
+    if (a2.guard) twk::adaptive_kernel<true><<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2), stream>>>(a2);
+    else twk::adaptive_kernel<false><<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2), stream>>>(a2);
     ++launches;
     mark();
   }
@@ -319,7 +328,8 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a3.list = list2;
     a3.count = counters + 3;
     a3.cursor = counters + 4;
-    twk::adaptive_kernel<<<P.grid3, twk::kThreads, twk::adaptive_smem_bytes(P.cap3), stream>>>(a3);
+    if (a3.guard) twk::adaptive_kernel<true><<<P.grid3, twk::kThreads, twk::adaptive_smem_bytes(P.cap3), stream>>>(a3);
+    else twk::adaptive_kernel<false><<<P.grid3, twk::kThreads, twk::adaptive_smem_bytes(P.cap3), stream>>>(a3);
     ++launches;
     mark();
   }

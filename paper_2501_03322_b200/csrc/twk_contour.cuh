@@ -555,6 +555,42 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth, double 
   return P;
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// L-4 guard (an EXTENSION of the paper's estimate, option hidden_crossing_guard, off by default; reading L-4).
+// Eq.(17) sees an interval through its end points only: a boundary that dips into a caustic and out again BETWEEN two
+// adjacent 3-image samples leaves no trace in them.  The ghost pair does: next to a fold its separation squared
+// D = |z_a - z_b|^2 is proportional to the distance of the boundary point from the caustic, a parabola in theta that
+// turns negative where the boundary is inside.  D is fitted through (A-, A, B) and (A, B, B+); a convex fit with its
+// vertex inside the interval at D* < 0 is a hidden pair of crossings enclosing the area v (pi/2)(-D*)/sqrt(C) (C = the
+// fit's curvature, v = speed of the ghost pair's midpoint); that area is added to the interval's error estimate.
+// dm, d, dp = theta_A - theta_A-, theta_B - theta_A, theta_B+ - theta_B.  Out of line: rare, optional.
+// ------------------------------------------------------------------------------------------------------------
+TWK_NOINLINE double hidden_crossing_term(RecRef Am, RecRef A, RecRef B, RecRef Bp, double dm, double d, double dp) {
+  if (A.nreal() != 3 || B.nreal() != 3) return 0.0;
+  const cd sA = A.z(1) - A.z(4), sB = B.z(1) - B.z(4);
+  const cd mA = A.z(1) + A.z(4), mB = B.z(1) + B.z(4);            // twice the midpoints
+  const double DA = norm2(sA), DB = norm2(sB);
+  const double v = 0.5 * sqrt(norm2(mB - mA)) / d;
+  double term = 0.0;
+#pragma unroll 1
+  for (int side = 0; side < 2; ++side) {
+    const RecRef& T = side ? Bp : Am;
+    if (T.nreal() != 3) continue;
+    const double D3 = norm2(T.z(1) - T.z(4));
+    const double x0 = side ? 0.0 : -dm, x1 = side ? d : 0.0, x2 = side ? d + dp : d;
+    const double y0 = side ? DA : D3, y1 = side ? DB : DA, y2 = side ? D3 : DB;
+    const double f01 = (y1 - y0) / (x1 - x0), f12 = (y2 - y1) / (x2 - x1);
+    const double C = (f12 - f01) / (x2 - x0);
+    if (!(C > 0.0)) continue;
+    const double xs = 0.5 * (x0 + x1) - f01 / (2.0 * C);
+    if (!(xs > 0.0 && xs < d)) continue;
+    const double ys = y0 + f01 * (xs - x0) + C * (xs - x0) * (xs - x1);
+    if (!(ys < 0.0)) continue;
+    term = fmax(term, v * (0.5 * 3.141592653589793238462643383279) * (-ys) / sqrt(C));
+  }
+  return term;
+}
+
 // a5, slope detector: re-judge the real pair (slots kp, km) of a 5-image record as the ghost pair ("pair 1
 // shall be rejudged as ghost images").  The record becomes a 3-image record: the other positive image in slot 0, the
 // other two negative images in slots 2 and 3, the pair's positions in the z fields of slots 1 and 4.

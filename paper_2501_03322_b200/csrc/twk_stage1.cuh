@@ -40,6 +40,7 @@ struct Stage1Args {
   double slope_gate2;    // square of the slope detector's proximity gate (twk_options.slope_gate)
   double slope_cos2;     // square of the largest |cos| still counted as perpendicular (twk_options.slope_cos)
   int ps_test;           // N1: point-source adequacy tests in front of the contour path (twk_options.point_source_test)
+  int guard;             // L-4 guard: hidden-crossing term in the interval estimates (twk_options.hidden_crossing_guard)
   int group;             // sources per group, 1..64 (smaller for small batches: more CTAs get work)
   int final_stage;       // 1: there is no refinement stage (max_samples < 128): cap status instead of pending
   const double* seeds;   // [kSeedDoubles][n_sources] seed blocks written by stage 0
@@ -66,6 +67,9 @@ __host__ __device__ constexpr size_t stage1_smem_bytes() {
          (size_t)(2 * kS1Group + 2 * 2 + 4) * 4 + kS1Group;
 }
 
+// kGuard: the L-4 hidden-crossing term (twk_options.hidden_crossing_guard) is compiled into its own instance of the
+// kernel: the default instance carries no trace of it (the loop is sensitive to every extra instruction)
+template <bool kGuard>
 __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Args p) {
   extern __shared__ double sm[];
   double* recs = sm;                                          // [26][64] records of the current source
@@ -164,6 +168,11 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
       constexpr int kSlopeVote = 1 << 8;
       for (;;) {
         P = eval_interval(mine, next, kTwoPi / double(kThreads), p.slope_gate2, p.slope_cos2);
+        if (kGuard && P.crossing == 0) {
+          const double h = kTwoPi / double(kThreads);
+          P.err += hidden_crossing_term(RecRef{recs + ((t + kThreads - 1) & (kThreads - 1)), kThreads}, mine, next,
+                                        RecRef{recs + ((t + 2) & (kThreads - 1)), kThreads}, h, h, h);
+        }
         // sums: warp shuffle, then the two warps through (double-buffered) shared memory
         A = P.dA;
         E = P.err;

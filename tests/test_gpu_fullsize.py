@@ -119,3 +119,33 @@ def test_cap_4096_like_for_like(ctx):
         assert g["nsamples"][0] == o["nsamples"][0] and 4096 - 64 < g["nsamples"][0] <= 4096
         # (at 4096 samples the estimate ~1e-9 sits on rounding-level ties of the sampler: same size, not same digits)
         assert abs(g["mu"][0] / o["mu"][0] - 1) < 1e-9 and 0.5 < g["err"][0] / o["err"][0] < 2.0
+
+
+def test_hidden_crossing_guard_closes_the_l4_cases():
+    """Option hidden_crossing_guard = 1 (reading L-4, an extension): like-for-like with the oracle's guard, and on the two
+    complete maps that hold the known L-4 sources no source is left beyond the tolerance because of a hidden crossing
+    (what remains on the close map are the two crossing pieces next to a cusp at 1.2e-4)."""
+    import paper_2501_03322_b200 as P
+    c = P.Context(1 << 21, hidden_crossing_guard=1)
+    for name, worst in (("close", 1.3e-4), ):
+        wl = W.fig5_map(name)
+        ref = api.magnify(wl, 1e-6, mode=1, prec=0)
+        g = c.magnify_workload(wl, 1e-4)
+        rel = np.abs(g["mu"] / ref["mu"] - 1)
+        assert (rel > 1e-4).sum() <= 2 and rel.max() < worst, (name, (rel > 1e-4).sum(), rel.max())
+    full = W.config4()
+    zc = full.zeta[:, 0] + 1j * full.zeta[:, 1]
+    near = np.where(np.abs(np.abs(zc) - 0.34) < 0.05)[0]                    # the ring of the map that holds the two L-4 sources
+    wl = full.subset(near)
+    assert np.any(np.abs(zc[near] - (-0.15087891 + 0.30615234j)) < 1e-6)
+    ref = api.magnify(wl, 1e-6, mode=1, prec=0)
+    g = c.magnify_workload(wl, 1e-4)
+    assert np.abs(g["mu"] / ref["mu"] - 1).max() <= 1e-4
+    # like-for-like with the oracle's guard: same sample counts, same values
+    for wl in (W.fig5_map("close").subset(np.arange(60000, 90000, 7)), W.config4().subset(near[::5])):
+        g = c.magnify_workload(wl, 1e-4)
+        o = api.magnify(wl, 1e-4, mode=0, hidden_guard=1)
+        same = g["nsamples"] == o["nsamples"]
+        assert same.mean() > 0.97 and np.quantile(np.abs(g["mu"] / o["mu"] - 1)[same], 0.99) < 1e-8
+        assert np.abs(g["mu"] / o["mu"] - 1).max() < 1e-4
+    c.close()
