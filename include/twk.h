@@ -59,7 +59,7 @@ typedef struct {
   int max_samples;      /* sample cap per source, default 4096; 64 <= max_samples <= 4096                  */
   int subtract_avg_tol; /* 1 = subtract the average tolerance from every interval error before sampling */
   int64_t handoff_slots; /* slots of the hand-over arena through which the first iteration (64 records, interval     */
-                        /* pieces, seeds; 14,592 B per slot) of an unfinished source passes to the refinement stage  */
+                        /* pieces, seeds; 14,720 B per slot) of an unfinished source passes to the refinement stage  */
                         /* instead of being recomputed there.  -1 = default min(max_sources, 524288); 0 = none.      */
                         /* Sources beyond the slots are still refined (their first iteration is recomputed).        */
   double slope_gate;    /* slope detector: at a change of the image count between adjacent samples the    */

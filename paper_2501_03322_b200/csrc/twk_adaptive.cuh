@@ -83,16 +83,36 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   };
   const long long total = p.count ? (long long)*p.count : p.b.n_sources;
 
+  // work fetch one source ahead: thread 0 takes the NEXT entry of the cursor at the start of the current source and
+  // publishes it at its end, so the atomic's round trip is never waited for
+  if (t == 0) iscr[0] = atomicAdd(p.cursor, 1);
   for (;;) {
-    __syncthreads();
-    if (t == 0) iscr[0] = atomicAdd(p.cursor, 1);
     __syncthreads();
     const long long cur = iscr[0];
     if (cur >= total) break;
-    const long long src = p.list ? (long long)p.list[cur] : cur;
+    int next_cur = 0;
+    if (t == 0) next_cur = atomicAdd(p.cursor, 1);
+    // a handed-over source starts from its slot's header; otherwise worklist -> model -> parameters
+    hand = (p.handoff && cur < p.handoff_slots) ? p.handoff + (size_t)cur * kHandDoubles : nullptr;
+    long long src;
+    SourceParams S;
+    if (hand) {
+      const double* hd = hand + kHandHeader;
+      src = __double_as_longlong(hd[0]);
+      S.L.s = hd[1];
+      S.L.m1 = hd[2];
+      S.L.m2 = hd[3];
+      S.L.z2 = hd[4];
+      S.zc = mk(hd[5], hd[6]);
+      S.rho = hd[7];
+      S.status = (uint32_t)code_of(hd[8]);
+      S.valid = true;
+    } else {
+      src = p.list ? (long long)p.list[cur] : cur;
+      S = load_source(p.b, src);
+    }
     TWK_CHECK(src >= 0 && src < p.b.n_sources, 4);
     if (t == 0) TWK_DEBUG_COUNT(6);
-    const SourceParams S = load_source(p.b, src);
     if (!S.valid) {
       if (t == 0) {
         p.out_mu[src] = nan("");
@@ -100,15 +120,16 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         if (p.out_nsamples) p.out_nsamples[src] = 0;
         if (p.out_status) p.out_status[src] = 8u;
       }
+      __syncthreads();
+      if (t == 0) iscr[0] = next_cur;
       continue;
     }
     // ---- first iteration: 64 uniform samples theta_j = 2 pi j / 64 (reading A-3) ----------------------
     int flags = 0;
     int n = 0;
-    hand = (p.handoff && cur < p.handoff_slots) ? p.handoff + (size_t)cur * kHandDoubles : nullptr;
     if (hand) {   // done by stage 1: take its interval pieces and seed block, use its records in place
-      // the slot was written long ago (4 GB of hand-over traffic per call has left the L2): pull its 14.6 KB back
-      // into the L2 now, the first solve hides the DRAM latency
+      // the slot was written long ago (4 GB of hand-over traffic per call has left the L2): pull its 14.7 KB back
+      // into the L2 now, the first solve hides the DRAM latency of the records
       {
         const char* hb = reinterpret_cast<const char*>(hand);
         asm volatile("prefetch.global.L2 [%0];" ::"l"(hb + t * 128));
@@ -381,6 +402,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
     const int nonf = __syncthreads_or(flags & (kPointNonFinite | kPointGuard));
     const int slp = __syncthreads_or(flags & kPointSlope);
     if (t == 0) {
+      iscr[0] = next_cur;   // (every thread read the current entry before the barriers above)
       if (exhausted && !p.final_stage) {
         const int slot = atomicAdd(p.next_count, 1);
         TWK_CHECK(slot >= 0 && slot < p.b.n_sources, 4);

@@ -47,8 +47,11 @@ constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr double kPi = 3.141592653589793238462643383279;
 constexpr double kInvPi = 0.318309886183790671537767526745;
 constexpr int kThreads = 64;   // threads per source = samples per iteration
-// Hand-over slot (stage 1 -> stage 2), in doubles: records [26][64] | dA [64] | err [64] | seed block [30] (+2 pad)
-constexpr int kHandDoubles = (kRecDoubles + 2) * kThreads + 32;
+// Hand-over slot (stage 1 -> stage 2), in doubles: records [26][64] | dA [64] | err [64] | seed block [31] (+1 pad) |
+// header [16]: source id (raw bits), s, m1, m2, z2, Re zc, Im zc, rho, status (raw bits) -- with the header the refinement
+// stage needs ONE round trip to memory to start a handed-over source (no worklist / model / parameter chain)
+constexpr int kHandHeader = (kRecDoubles + 2) * kThreads + 32;
+constexpr int kHandDoubles = kHandHeader + 16;
 
 struct Batch {
   const double* s;

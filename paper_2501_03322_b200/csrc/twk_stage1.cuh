@@ -235,6 +235,11 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
           h[kRecDoubles * kThreads + t] = P.dA;
           h[(kRecDoubles + 1) * kThreads + t] = P.err;
           if (t < kSeedDoubles) h[(kRecDoubles + 2) * kThreads + t] = seeds[t * kS1Group + i];
+          if (t >= 32 && t < 32 + 9) {   // header: what stage 2 needs to start this source without looking anything up
+            const int k = t - 32;
+            h[kHandHeader + k] = (k == 0) ? __longlong_as_double(base + i)
+                                          : (k == 8) ? code_as_double(code & 255) : prm[(k - 1) * kS1Group + i];
+          }
         }
       }
       if (t == 0) {

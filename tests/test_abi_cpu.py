@@ -29,9 +29,9 @@ def test_workspace_bytes_is_host_arithmetic():
     a = P.twk_workspace_bytes(1000)
     b = P.twk_workspace_bytes(4096000)
     assert 0 < a < b < 1 << 34
-    # the hand-over arena (14,592 B per slot, default min(max_sources, 2^19) slots) is the bulk of a large context
+    # the hand-over arena (14,720 B per slot, default min(max_sources, 2^19) slots) is the bulk of a large context
     lean = P.twk_workspace_bytes(4096000, handoff_slots=0)
-    assert lean < 1 << 31 and b - lean == (1 << 19) * 14592
+    assert lean < 1 << 31 and b - lean == (1 << 19) * 14720
     assert P.twk_workspace_bytes(1000, handoff_slots=-2) == 0        # invalid
     assert P.twk_workspace_bytes(1000, max_samples=512) < a          # no stage-3 arena
     assert P.twk_workspace_bytes(1000, max_samples=5000) == 0        # invalid options
