@@ -62,6 +62,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true")
     ap.add_argument("--profile-pass", action="store_true")
+    ap.add_argument("--pass-workloads", default=None, help="comma list restricting --profile-pass (default: all)")
     ap.add_argument("--parse-ncu", default=None)
     ap.add_argument("--scaling", action="store_true")
     return ap.parse_args()
@@ -311,7 +312,7 @@ def main():
     dev = torch.device("cuda", local)
 
     if args.profile_pass:                   # what the ncu counting pass runs: one call per workload, nothing else
-        for name in ["config3"] + OTHER:
+        for name in (args.pass_workloads.split(",") if args.pass_workloads else ["config3"] + OTHER):
             wl = make_workload(name)
             ctx = P.Context(wl.n_sources)
             d = ctx.upload(wl, dev)
