@@ -39,15 +39,23 @@ struct AdaptArgs {
   uint32_t* out_status;  // may be null
 };
 
-__host__ __device__ inline size_t adaptive_smem_bytes(int cap) {
-  size_t doubles = 3 * (size_t)cap + 2 * kThreads + 8 + 32;
+constexpr int kScrDoubles = 20;   // per-thread scratch of point_solve_cs<true> (roots and residuals of the five roots)
+__host__ __device__ inline size_t adaptive_smem_bytes(int cap, bool scr, bool tile) {
+  // (with a tile the scratch of the point solves is the tile column the record goes to)
+  size_t doubles = 3 * (size_t)cap + 2 * kThreads + 8 + 32 + (scr && !tile ? kScrDoubles * kThreads : 0) + (tile ? kRecDoubles * kThreads : 0);
   size_t ints = 2 * kThreads + 4;
   return doubles * 8 + ints * 4 + (size_t)cap * 2;
 }
 
 // 6 CTAs per SM (168 registers): measured 4 / 5 / 6 / 8 CTAs per SM on configs 3 and 5: 9.4 / 9.3 / 8.6 / 8.8 ms and
 // 7.6 / 7.4 / 6.7 / 7.0 ms -- the kernel is latency-bound and wants warps, but at 128 registers it spills
-template <bool kGuard>   // the L-4 hidden-crossing term lives in its own instance of the kernel (see stage1_kernel)
+// kGuard: the L-4 hidden-crossing term lives in its own instance of the kernel (see stage1_kernel)
+// kScr:   [20][64] doubles of shared-memory scratch for the residual detector (stage 2; at the 4096-sample capacity of
+//         stage 3 the 10 KB would cost the second resident CTA, so that instance selects in registers)
+// kTile:  the records of the iteration's NEW samples are written twice, to the arena (where later iterations find them) and
+//         to a [26][64] shared-memory tile; the interval evaluations of the same iteration read every new record -- each
+//         thread's own, above all -- from the tile instead of waiting for the arena
+template <bool kGuard, bool kScr, bool kTile>
 __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   extern __shared__ double sm[];
   const int cap = p.cap;
@@ -58,7 +66,9 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   double* cth = newth + kThreads;   // [64] compacted new angles
   double* scratch = cth + kThreads; // [8]
   double* seeds = scratch + 8;      // [30 (+2)] seed block of the source (twk_contour.cuh)
-  int* newint = reinterpret_cast<int*>(seeds + 32);   // [64] interval of quantile k
+  double* scrbuf = seeds + 32;      // [20][64] (kScr) scratch of the point solves
+  double* tile = scrbuf + (kScr && !kTile ? kScrDoubles * kThreads : 0);   // [26][64] (kTile) records of this iteration's new samples
+  int* newint = reinterpret_cast<int*>(tile + (kTile ? kRecDoubles * kThreads : 0));   // [64] interval of quantile k
   int* cint = newint + kThreads;    // [64] compacted
   int* iscr = cint + kThreads;      // [4]
   uint16_t* ids = reinterpret_cast<uint16_t*>(iscr + 4);   // [cap] arena id of the sample at each sorted position
@@ -68,8 +78,10 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   double* arena = p.arena + (size_t)blockIdx.x * (size_t)cap * kRecDoubles;
   // record of sample id: ids 0..63 of a handed-over source live in its hand-over slot ([26][64]), the rest in the arena
   const double* hand = nullptr;
+  int tile_base = 1 << 30;   // ids >= tile_base are in the tile (the current iteration's new samples)
   auto recref = [&](int id) -> RecRef {
     TWK_CHECK(id >= 0 && id < cap, 0);
+    if (kTile && id >= tile_base) return RecRef{tile + (id - tile_base), kThreads};
     if (hand && id < kThreads) return RecRef{const_cast<double*>(hand) + id, kThreads};
     return RecRef{arena + (size_t)id * kRecDoubles, 1};
   };
@@ -297,9 +309,12 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         double sn, cs;
         if (n == 0) sincospi(double(t) / 32.0, &sn, &cs);   // exactly stage 1's angles
         else sincospi(th * kInvPi, &sn, &cs);               // no range-reduction slow path
-        flags |= point_solve_cs(S.L, S.zc, S.rho, cs, sn, seeds, 1, recref(n + t), nullptr, nullptr, nullptr);
+        const RecRef in_arena{arena + (size_t)(n + t) * kRecDoubles, 1};
+        flags |= point_solve_cs<kScr, kTile>(S.L, S.zc, S.rho, cs, sn, seeds, 1, kTile ? RecRef{tile + t, kThreads} : in_arena,
+                                             nullptr, nullptr, nullptr, RecRef{(kTile ? tile : scrbuf) + t, kThreads}, in_arena);
       }
       const int n_new = n + m;
+      tile_base = kTile ? n : (1 << 30);
       __syncthreads();
 #ifdef TWK_DEBUG
       {   // the sorted list after the merge: angles strictly increasing, ids a permutation of 0 .. n_new - 1
@@ -346,6 +361,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
       //      five images). ------------------------------------------------------------------------------------------
       if (__syncthreads_or(viol)) {
         slope_seen = true;
+        tile_base = 1 << 30;   // the repair rounds change records: from here on only the arena's copies are used
         for (int round = 0; round < 4096; ++round) {
           if (t == 0) iscr[3] = 0;
           __syncthreads();

@@ -12,6 +12,9 @@
 namespace {
 
 constexpr int kAssumedSMs = 148;        // B200; workspace sizing only (twk_workspace_bytes needs no GPU)
+// stage 2 keeps this iteration's new records in a shared-memory tile next to the arena (the tile column doubles as the
+// scratch of the point solve); at the 4096-sample capacity of stage 3 the tile would cost the second resident CTA
+constexpr bool kStage2Scr = true, kStage2Tile = true;
 constexpr int kStage2Cap = 512;         // sample capacity of refinement stage 2
 constexpr int kStage2CtasPerSM = 6;
 constexpr int kStage3CtasPerSM = 2;
@@ -179,11 +182,11 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   }
   // opt in to the large dynamic shared memory of stage 3 (a per-function attribute shared by all contexts, so
   // always the maximum the build supports)
-  e = cudaFuncSetAttribute(twk::adaptive_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)twk::adaptive_smem_bytes(4096));
+  e = cudaFuncSetAttribute(twk::adaptive_kernel<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)twk::adaptive_smem_bytes(4096, false, false));
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(twk::adaptive_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)twk::adaptive_smem_bytes(4096));
+    e = cudaFuncSetAttribute(twk::adaptive_kernel<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)twk::adaptive_smem_bytes(4096, false, false));
   if (e != cudaSuccess) {
     cudaFree(c->ws);
     delete c;
@@ -316,8 +319,10 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a2.next_count = counters + 3;
     a2.handoff = handoff;
     a2.handoff_slots = (long long)ctx->lay.slots;
-    if (a2.guard) twk::adaptive_kernel<true><<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2), stream>>>(a2);
-    else twk::adaptive_kernel<false><<<P.grid2, twk::kThreads, twk::adaptive_smem_bytes(P.cap2), stream>>>(a2);
+    constexpr bool kScr2 = kStage2Scr, kTile2 = kStage2Tile;
+    const size_t smem2 = twk::adaptive_smem_bytes(P.cap2, kScr2, kTile2);
+    if (a2.guard) twk::adaptive_kernel<true, kScr2, kTile2><<<P.grid2, twk::kThreads, smem2, stream>>>(a2);
+    else twk::adaptive_kernel<false, kScr2, kTile2><<<P.grid2, twk::kThreads, smem2, stream>>>(a2);
     ++launches;
     mark();
   }
@@ -328,8 +333,9 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a3.list = list2;
     a3.count = counters + 3;
     a3.cursor = counters + 4;
-    if (a3.guard) twk::adaptive_kernel<true><<<P.grid3, twk::kThreads, twk::adaptive_smem_bytes(P.cap3), stream>>>(a3);
-    else twk::adaptive_kernel<false><<<P.grid3, twk::kThreads, twk::adaptive_smem_bytes(P.cap3), stream>>>(a3);
+    const size_t smem3 = twk::adaptive_smem_bytes(P.cap3, false, false);
+    if (a3.guard) twk::adaptive_kernel<true, false, false><<<P.grid3, twk::kThreads, smem3, stream>>>(a3);
+    else twk::adaptive_kernel<false, false, false><<<P.grid3, twk::kThreads, smem3, stream>>>(a3);
     ++launches;
     mark();
   }

@@ -83,8 +83,15 @@ TWK_HD bool lens_guard(cd& y, double s) {
 // centre_seeds() (element e at seeds[e * seed_stride]): every root of the boundary sample is predicted to first order
 // from the centre's root, eta_k + A_k delta + B_k conj(delta) with delta = rho e^{i theta}, and refined by the seeded
 // Newton solve, with the cold solver as verified fallback.
+// kScr: `scr` is per-thread scratch of >= 20 elements in SHARED memory (it may be the record itself: the scratch is dead
+// before the record is written).  The residual detector then parks the roots and their residuals there and fetches the
+// two largest-|R| ones by index: 28 shared-memory accesses instead of ~140 register selects.
+// kDual: the record is also written to `rec2` (the refinement kernel keeps a shared-memory copy of the new records
+// next to the arena's).
+template <bool kScr = false, bool kDual = false>
 TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn, const double* seeds, int seed_stride,
-                          RecRef rec, double* out_z, int8_t* out_kind, int8_t* out_count) {
+                          RecRef rec, double* out_z, int8_t* out_kind, int8_t* out_count, RecRef scr = RecRef{nullptr, 0},
+                          RecRef rec2 = RecRef{nullptr, 0}) {
   const cd zeta = mk(fma(rho, cs, zc.x), fma(rho, sn, zc.y));
   const cd dzeta = mk(-rho * sn, rho * cs);                     // zeta' = i rho e^{i theta}
   cd y = mk(zeta.x - L.z2, zeta.y);
@@ -105,6 +112,12 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
       const double bx = seeds[(20 + k) * seed_stride], by = seeds[(25 + k) * seed_stride];
       // A delta + B conj(delta)
       eta[k] = mk(ex + fma(ax + bx, dx, (by - ay) * dy), ey + fma(ay + by, dx, (ax - bx) * dy));
+    }
+    {   // the seeded solve works on the monic quintic; the cold solver below gets the same coefficients with c5 = 1
+      const cd i5 = crecip(c[5]);
+#pragma unroll
+      for (int i = 0; i < 5; ++i) c[i] = c[i] * i5;
+      c[5] = mk(1.0, 0.0);
     }
     solved = quintic_roots_seeded(c, eta, seeds[30 * seed_stride] != 0.0);
   }
@@ -144,13 +157,37 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   int ia = 0, ib = -1;
   double mA = R2[0], mB = -1.0;
   cd eA = eta[0], rA = Res[0], eB = eta[0], rB = Res[0];
+  if (kScr) {
 #pragma unroll
-  for (int k = 1; k < 5; ++k) {
-    if (R2[k] > mA) {          // new largest: the old largest becomes the second
-      mB = mA; ib = ia; eB = eA; rB = rA;
-      mA = R2[k]; ia = k; eA = eta[k]; rA = Res[k];
-    } else if (R2[k] > mB) {
-      mB = R2[k]; ib = k; eB = eta[k]; rB = Res[k];
+    for (int k = 0; k < 5; ++k) {
+      scr.at(k) = eta[k].x;
+      scr.at(5 + k) = eta[k].y;
+      scr.at(10 + k) = Res[k].x;
+      scr.at(15 + k) = Res[k].y;
+    }
+#pragma unroll
+    for (int k = 1; k < 5; ++k) {
+      if (R2[k] > mA) {
+        mB = mA; ib = ia;
+        mA = R2[k]; ia = k;
+      } else if (R2[k] > mB) {
+        mB = R2[k]; ib = k;
+      }
+    }
+    const int jb = ib < 0 ? 0 : ib;   // (only when every |R| is NaN)
+    eA = mk(scr.at(ia), scr.at(5 + ia));
+    rA = mk(scr.at(10 + ia), scr.at(15 + ia));
+    eB = mk(scr.at(jb), scr.at(5 + jb));
+    rB = mk(scr.at(10 + jb), scr.at(15 + jb));
+  } else {
+#pragma unroll
+    for (int k = 1; k < 5; ++k) {
+      if (R2[k] > mA) {          // new largest: the old largest becomes the second
+        mB = mA; ib = ia; eB = eA; rB = rA;
+        mA = R2[k]; ia = k; eA = eta[k]; rA = Res[k];
+      } else if (R2[k] > mB) {
+        mB = R2[k]; ib = k; eB = eta[k]; rB = Res[k];
+      }
     }
   }
   const cd dab = eB - eA;
@@ -203,6 +240,13 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
       rec.at(kPX + slot) = zp.x;
       rec.at(kPY + slot) = zp.y;
       rec.at(kW + slot) = w;
+      if (kDual) {
+        rec2.at(kZX + slot) = z.x;
+        rec2.at(kZY + slot) = z.y;
+        rec2.at(kPX + slot) = zp.x;
+        rec2.at(kPY + slot) = zp.y;
+        rec2.at(kW + slot) = w;
+      }
     }
   }
   if (nreal == 3) {   // ghost pair positions for the slope detector
@@ -210,8 +254,15 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     rec.at(kZY + 1) = eA.y;
     rec.at(kZX + 4) = eB.x + L.z2;
     rec.at(kZY + 4) = eB.y;
+    if (kDual) {
+      rec2.at(kZX + 1) = eA.x + L.z2;
+      rec2.at(kZY + 1) = eA.y;
+      rec2.at(kZX + 4) = eB.x + L.z2;
+      rec2.at(kZY + 4) = eB.y;
+    }
   }
   rec.set_code(nreal + 8 * flags);
+  if (kDual) rec2.set_code(nreal + 8 * flags);
   if (out_count) *out_count = (int8_t)nreal;
   return flags;
 }

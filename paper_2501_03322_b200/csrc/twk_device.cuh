@@ -66,6 +66,18 @@ TWK_HD double rcp(double x) {
   return 1.0 / x;
 #endif
 }
+// 1/x to ~40 bits: the estimate + ONE Newton step.  For Newton corrections only (a relative error of 1e-12 in a step
+// that is itself <= 1e-4 of the root is far below the rounding of the root).
+TWK_HD double rcp1(double x) {
+#ifdef __CUDA_ARCH__
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+#else
+  return 1.0 / x;
+#endif
+}
 TWK_HD cd crecip(cd a) {
   const double inv = rcp(norm2(a));
   return mk(a.x * inv, -a.y * inv);
@@ -267,7 +279,7 @@ TWK_NOINLINE Roots5 quintic_roots_cold(Coef6 C) {
 // with the rounding floor of its own evaluation (ill-conditioned roots next to a caustic stall there).
 // Verification: all five converged and distinct (Vieta: sum of roots = -c4/c5).
 // Recovery (at most once per solve): when two chains ran into the same root, or up to two chains have not
-// converged after 10 sweeps, the three or four good distinct roots fix the others through Vieta's formulas
+// converged after TWK_RECOVER_AT (4) sweeps, the three or four good distinct roots fix the others through Vieta's formulas
 // (sum of roots = -c4/c5, product = -c0/c5: one missing root directly, two as the roots of a quadratic); these
 // are polished by the same Newton sweeps and the verification is repeated.
 // Returns 0 when that fails too; the caller then falls back to the cold solver quintic_roots().
@@ -275,6 +287,9 @@ TWK_NOINLINE Roots5 quintic_roots_cold(Coef6 C) {
 // Two converged chains are the same root when they agree to 1e-6 of their size (RELATIVE: next to a planet of
 // q = 1e-9 two distinct roots can be 1e-9 apart in absolute terms while the other roots are of order one).
 constexpr double kDupRel2 = 1e-12;
+#ifndef TWK_RECOVER_AT
+#define TWK_RECOVER_AT 4   // sweeps before chains that have not converged are replaced through Vieta's formulas
+#endif
 
 struct SeededState {
   cd r[5];
@@ -329,27 +344,35 @@ TWK_NOINLINE SeededState seeded_recover(cd c0, cd c5, cd tot, SeededState S) {
 // One Newton step of root x on the quintic c.  kFloor: also compare the residual with the rounding floor of its own
 // evaluation.  Returns true when the root is converged (see the stop rule above); prev = |dx| of the previous step.
 template <bool kFloor>
-TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev) {
+TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev, bool check = true) {
   TWK_COUNT(newton_eval);
-  cd p = cfma(c[5], x, c[4]), d = c[5];      // Horner for p and p', first step peeled (p' starts from c5, not from 0)
+  // c[0..4] are the coefficients of the MONIC quintic (c[5] is not read): the first two Horner steps are additions
+  cd p = mk(x.x + c[4].x, x.y + c[4].y);
+  cd d = mk(x.x + p.x, x.y + p.y);
+  p = cfma(p, x, c[3]);
 #pragma unroll
-  for (int i = 3; i >= 0; --i) {
+  for (int i = 2; i >= 0; --i) {
     d = cfma(d, x, p);
     p = cfma(p, x, c[i]);
   }
   if (kFloor) {
     const double ax = abs1(x);
-    double err = abs1(c[5]);
+    double err = 1.0;
 #pragma unroll
     for (int i = 4; i >= 0; --i) err = fma(err, ax, abs1(c[i]));
     if (abs1(p) <= 2.0 * kEps * err) return true;   // at the rounding floor
   }
   const double dn = norm2(d);
   if (!(dn > 0.0)) return false;
-  const cd dx = cdiv(p, d);
+  const double inv = rcp1(dn);
+  const cd dx = mk(fma(p.x, d.x, p.y * d.y) * inv, fma(p.y, d.x, -(p.x * d.y)) * inv);
   x = x - dx;
-  const double sdx = abs1(dx), ar = abs1(x);
-  const bool conv = sdx * sdx * sdx <= (TWK_STOP_FACTOR * kEps) * ar * prev * prev || sdx <= kEps * ar;
+  const double sdx = abs1(dx);
+  bool conv = false;
+  if (check) {   // (the first sweep of a solve has no previous step: only a later one can satisfy the rule)
+    const double ar = abs1(x);
+    conv = sdx * sdx * sdx <= (TWK_STOP_FACTOR * kEps) * ar * prev * prev || sdx <= kEps * ar;
+  }
   prev = sdx;
   return conv;
 }
@@ -359,7 +382,7 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
   double prev[5];
 #pragma unroll
   for (int k = 0; k < 5; ++k) prev[k] = 0.0;
-  const cd tot = -cdiv(c[4], c[5]);   // sum of the five roots
+  const cd tot = -c[4];               // sum of the five roots (monic coefficients)
   unsigned done = 0;
   // sweeps 0 and 1: every root needs them (the stop rule wants two steps), so all five chains run unconditionally
   // and interleave (instruction-level parallelism); a step on an already converged root is harmless
@@ -368,12 +391,12 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
   for (int it = 0; it < 2; ++it) {
     unsigned dn = 0;
 #pragma unroll
-    for (int k = 0; k < 5; ++k) dn |= newton_step<false>(c, r[k], prev[k]) ? (1u << k) : 0u;
+    for (int k = 0; k < 5; ++k) dn |= newton_step<false>(c, r[k], prev[k], it != 0) ? (1u << k) : 0u;
     done |= dn;
   }
   bool recovered = false;
   for (int it = 2; it < 22; ++it) {
-    if (done == 31u || (it >= 10 && !recovered)) {
+    if (done == 31u || (it >= TWK_RECOVER_AT && !recovered)) {
       if (done == 31u) {
         // verification by Vieta: the sum of the roots (absolute, on the scale of the largest) and, for sources
         // flagged by centre_seeds (two roots closer than 1e-6 of the scale: next to a q = 1e-9 planet two chains on
@@ -386,7 +409,7 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
         // to any duplicate when one root has run off towards infinity (a sample next to a lens)
         {
           const cd prod = ((r[0] * r[1]) * (r[2] * r[3])) * r[4];
-          ok = ok && abs1(prod * c[5] + c[0]) <= 1e-9 * abs1(c[0]);          // prod = -c0/c5
+          ok = ok && abs1(prod + c[0]) <= 1e-9 * abs1(c[0]);                 // prod = -c0 (monic)
         }
         (void)check_product;
         if (ok) return recovered ? 2 : 1;
@@ -398,7 +421,7 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
       for (int k = 0; k < 5; ++k) S.r[k] = r[k];
       S.done = done;
       S.ok = 0;
-      S = seeded_recover(c[0], c[5], tot, S);
+      S = seeded_recover(c[0], mk(1.0, 0.0), tot, S);
       if (!S.ok) break;
 #pragma unroll
       for (int k = 0; k < 5; ++k)

@@ -160,8 +160,8 @@ __global__ void __launch_bounds__(TILE) fixed_kernel(Batch b, int N, double* __r
         const size_t o = (size_t)src * N + j;
         double sn, cs;
         sincos(kTwoPi * double(j) / double(N), &sn, &cs);
-        flags = point_solve_cs(S.L, S.zc, S.rho, cs, sn, SEEDED ? seeds : nullptr, 1, mine, out_z ? out_z + o * 10 : nullptr,
-                               out_kind ? out_kind + o * 5 : nullptr, out_count ? out_count + o : nullptr);
+        flags = point_solve_cs<true>(S.L, S.zc, S.rho, cs, sn, SEEDED ? seeds : nullptr, 1, mine, out_z ? out_z + o * 10 : nullptr,
+                                     out_kind ? out_kind + o * 5 : nullptr, out_count ? out_count + o : nullptr, mine);
       }
       if (SEEDED && diag) {
         const unsigned act = __ballot_sync(0xffffffffu, j < N), rcv = __ballot_sync(0xffffffffu, flags & kPointRecovered),

@@ -115,8 +115,13 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
         prm[6 * kS1Group + t] = S.rho;
         int code = (int)S.status | (S.valid ? 256 : 0);
         if (S.valid) {
-#pragma unroll 1
-          for (int e = 0; e < kSeedDoubles; ++e) seeds[e * kS1Group + t] = p.seeds[(size_t)e * (size_t)n + (size_t)src];
+          {   // all 31 loads in flight at once (one DRAM latency per group, not 31)
+            double sv[kSeedDoubles];
+#pragma unroll
+            for (int e = 0; e < kSeedDoubles; ++e) sv[e] = __ldg(p.seeds + (size_t)e * (size_t)n + (size_t)src);
+#pragma unroll
+            for (int e = 0; e < kSeedDoubles; ++e) seeds[e * kS1Group + t] = sv[e];
+          }
           if (p.ps_test) {   // N1: quadrupole + ghost-image tests; adequate -> no contour for this source
             const PsResult r = point_source_adequate_cold(S.L, S.zc, S.rho, seeds + t, kS1Group, p.tol);
             if (r.ok) {
@@ -151,7 +156,7 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
       L.z2 = prm[3 * kS1Group + i];
       const cd zc = mk(prm[4 * kS1Group + i], prm[5 * kS1Group + i]);
       const double rho = prm[6 * kS1Group + i];
-      int flags = point_solve_cs(L, zc, rho, cs, sn, seeds + i, kS1Group, mine, nullptr, nullptr, nullptr);
+      int flags = point_solve_cs<true>(L, zc, rho, cs, sn, seeds + i, kS1Group, mine, nullptr, nullptr, nullptr, mine);
       if (p.diag) {
         const unsigned rec = __ballot_sync(0xffffffffu, flags & kPointRecovered), cold = __ballot_sync(0xffffffffu, flags & kPointCold),
                        grd = __ballot_sync(0xffffffffu, flags & kPointGuard);
