@@ -299,6 +299,22 @@ TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int st
 #pragma unroll
     for (int k = 0; k < 5; ++k) eta[k] = R.r[k];
   }
+  {   // the root of largest modulus goes last: the seeded solve derives the fifth root from Vieta's sum (twk_device.cuh)
+    int big = 0;
+    double nb = norm2(eta[0]);
+#pragma unroll
+    for (int k = 1; k < 5; ++k)
+      if (norm2(eta[k]) > nb) { nb = norm2(eta[k]); big = k; }
+    const cd last = eta[4];
+    cd e = eta[0];
+#pragma unroll
+    for (int k = 1; k < 5; ++k)
+      if (k == big) e = eta[k];
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (k == big) eta[k] = last;
+    eta[4] = e;
+  }
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
     const cd a = crecip(mk(-L.s - eta[k].x, -eta[k].y));
@@ -453,20 +469,32 @@ struct Piece {
                   // ghost pair next to it and must be re-judged: slot of its positive image | slot of its negative << 4 | 256
 };
 
-TWK_HD void link_terms(const RecRef& A, const RecRef& B, int ka, int kb, double par, double dth, double& dA,
+// the powers of the interval's width that every link of the interval uses (computed once per interval)
+struct LinkConst {
+  double dth2, c24, c12, c48;   // dth^2, dth^3/24, dth/12, dth^3/48
+};
+TWK_HD LinkConst link_const(double dth) {
+  LinkConst K;
+  K.dth2 = dth * dth;
+  const double dth3 = K.dth2 * dth;
+  K.c24 = dth3 * (1.0 / 24.0);
+  K.c12 = dth * (1.0 / 12.0);
+  K.c48 = dth3 * (1.0 / 48.0);
+  return K;
+}
+TWK_HD void link_terms(const RecRef& A, const RecRef& B, int ka, int kb, double par, const LinkConst& K, double& dA,
                        double& err) {
   const cd zA = A.z(ka), zB = B.z(kb), pA = A.zp(ka), pB = B.zp(kb);
   const double wA = A.w(ka), wB = B.w(kb);
   const cd dz = zB - zA;
-  const double dth2 = dth * dth, dth3 = dth2 * dth;
   const double trap = 0.5 * wedge(zA, dz);                              // Eq.(9)
-  const double p1 = (wA + wB) * dth3 * (1.0 / 24.0);                    // Eq.(10) dA^(p1)
-  const double p2 = wedge(dz, pB - pA) * dth * (1.0 / 12.0);            // Eq.(10) dA^(p2)
+  const double p1 = (wA + wB) * K.c24;                                  // Eq.(10) dA^(p1)
+  const double p2 = wedge(dz, pB - pA) * K.c12;                         // Eq.(10) dA^(p2)
   const double dAp = 0.5 * (p1 + p2);
   dA += par * (trap + dAp);
-  const double E1 = fabs(wA - wB) * dth3 * (1.0 / 48.0);                // Eq.(17)
-  const double E2 = 1.5 * fabs(dAp * (norm2(dz) * rcp(dth2 * fabs(dotp(pA, pB))) - 1.0));
-  const double E3 = 0.1 * fabs(dAp) * dth2;
+  const double E1 = fabs(wA - wB) * K.c48;                              // Eq.(17)
+  const double E2 = 1.5 * fabs(dAp * (norm2(dz) * rcp1(K.dth2 * fabs(dotp(pA, pB))) - 1.0));   // (an estimate: 40 bits do)
+  const double E3 = 0.1 * fabs(dAp) * K.dth2;
   const double E4 = fabs(p1 - p2);
   err += (E1 + E2) + (E3 + E4);
 }
@@ -560,11 +588,12 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth, double 
     }
   }
   // ---- a7: area and error of every link (one copy of the code; 3 or 4 or 5 trips) ----------------------------
+  const LinkConst K = link_const(dth);
 #pragma unroll 1
   for (int l = 0; l < nl; ++l) {
     const int ka = (int)(links & 15u), kb = (int)((links >> 4) & 15u);
     links >>= 8;
-    link_terms(A, B, ka, kb, ka < 2 ? 1.0 : -1.0, dth, P.dA, P.err);
+    link_terms(A, B, ka, kb, ka < 2 ? 1.0 : -1.0, K, P.dA, P.err);
   }
   // ---- caustic crossing: the extra (+,-) pair on the 5-image side connects to itself -------------
   if (a5 != b5) {

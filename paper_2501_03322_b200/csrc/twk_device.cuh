@@ -363,15 +363,15 @@ TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev, bool check = true
     if (abs1(p) <= 2.0 * kEps * err) return true;   // at the rounding floor
   }
   const double dn = norm2(d);
-  if (!(dn > 0.0)) return false;
-  const double inv = rcp1(dn);
+  const bool slope = dn > 0.0;               // p' = 0 (or NaN): no step, not converged -- as selects, not as a branch
+  const double inv = slope ? rcp1(dn) : 0.0;
   const cd dx = mk(fma(p.x, d.x, p.y * d.y) * inv, fma(p.y, d.x, -(p.x * d.y)) * inv);
   x = x - dx;
   const double sdx = abs1(dx);
   bool conv = false;
   if (check) {   // (the first sweep of a solve has no previous step: only a later one can satisfy the rule)
     const double ar = abs1(x);
-    conv = sdx * sdx * sdx <= (TWK_STOP_FACTOR * kEps) * ar * prev * prev || sdx <= kEps * ar;
+    conv = slope && (sdx * sdx * sdx <= (TWK_STOP_FACTOR * kEps) * ar * prev * prev || sdx <= kEps * ar);
   }
   prev = sdx;
   return conv;
@@ -391,22 +391,35 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
   for (int it = 0; it < 2; ++it) {
     unsigned dn = 0;
 #pragma unroll
-    for (int k = 0; k < 5; ++k) dn |= newton_step<false>(c, r[k], prev[k], it != 0) ? (1u << k) : 0u;
+    for (int k = 0; k < 4; ++k) dn |= newton_step<false>(c, r[k], prev[k], it != 0) ? (1u << k) : 0u;
     done |= dn;
   }
+  // The FIFTH root is not iterated: it follows from Vieta's sum, r4 = -c4 - (r0 + r1 + r2 + r3).  centre_seeds() puts the
+  // root of largest modulus last, so the rounding of the sum (a few ulp of the LARGEST root) is a relative error of
+  // a few ulp of r4 itself; the product of the five roots then verifies the solve.  v5 = that short cut is still on
+  // (bit 4 of `done` is preset); it is dropped -- and chain 4 iterated from its seed like the others -- as soon as
+  // something does not converge or verify.
+  bool v5 = true;
+  done |= 16u;
+  int rec_at = TWK_RECOVER_AT;
   bool recovered = false;
-  for (int it = 2; it < 22; ++it) {
-    if (done == 31u || (it >= TWK_RECOVER_AT && !recovered)) {
+  for (int it = 2; it < 24; ++it) {
+    if (v5 && done != 31u && it >= rec_at) {   // a chain is slow: give the recovery all five chains to choose from
+      v5 = false;
+      done &= 15u;
+      rec_at = it + 3;
+    }
+    if (done == 31u || (it >= rec_at && !recovered)) {
       if (done == 31u) {
-        // verification by Vieta: the sum of the roots (absolute, on the scale of the largest) and, for sources
-        // flagged by centre_seeds (two roots closer than 1e-6 of the scale: next to a q = 1e-9 planet two chains on
-        // one of two tiny neighbouring roots change the sum by 1e-9 of its scale, below this test), their product
-        // (relative)
-        const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
-        bool ok = abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale;
-        // ... and ALWAYS the product (relative): the sum alone is blind to two duplicated chains whose errors cancel (a
-        // sample at a symmetric point: equal masses, zeta = 0), to a duplicate among roots 1e-9 of the scale apart, and
-        // to any duplicate when one root has run off towards infinity (a sample next to a lens)
+        if (v5) r[4] = tot - ((r[0] + r[1]) + (r[2] + r[3]));
+        // verification by Vieta: the product of the roots (relative) catches two chains on one root -- also where the sum
+        // is blind (a symmetric sample: equal masses, zeta = 0; roots 1e-9 of the scale apart next to a tiny planet; a
+        // root that has run off towards infinity) -- and, when all five were iterated, the sum (on the scale of the largest)
+        bool ok = true;
+        if (!v5) {
+          const double scale = abs1(r[0]) + abs1(r[1]) + abs1(r[2]) + abs1(r[3]) + abs1(r[4]);
+          ok = abs1((r[0] + r[1]) + (r[2] + r[3]) + r[4] - tot) <= 1e-9 * scale;
+        }
         {
           const cd prod = ((r[0] * r[1]) * (r[2] * r[3])) * r[4];
           ok = ok && abs1(prod + c[0]) <= 1e-9 * abs1(c[0]);                 // prod = -c0 (monic)
@@ -419,7 +432,8 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
       SeededState S;
 #pragma unroll
       for (int k = 0; k < 5; ++k) S.r[k] = r[k];
-      S.done = done;
+      S.done = v5 ? (done & 15u) : done;   // (a Vieta-derived r4 is not evidence)
+      v5 = false;
       S.ok = 0;
       S = seeded_recover(c[0], mk(1.0, 0.0), tot, S);
       if (!S.ok) break;
