@@ -270,18 +270,22 @@ TWK_NOINLINE Roots5 quintic_roots_cold(Coef6 C) {
   return R;
 }
 
-// Seeded solve: Newton iteration on the ORIGINAL quintic for all five roots at once (five independent chains),
-// started from predictions of the roots (centre_seeds() in twk_contour.cuh).  Roots of a polynomial are continuous
-// in its coefficients, so ghosts can be followed like real images.
+// Seeded solve: Newton iteration on the MONIC quintic (the caller divides the coefficients by c5), four independent
+// chains at once, started from predictions of the roots (centre_seeds() in twk_contour.cuh).  Roots of a polynomial are
+// continuous in its coefficients, so ghosts can be followed like real images.  The FIFTH root -- the one of largest
+// modulus, which centre_seeds() orders last -- is not iterated: it follows from Vieta's sum, r4 = -c4 - (r0+r1+r2+r3).
 // Stop rule per root: Newton converges quadratically, |dx_{n+1}| ~ K |dx_n|^2 with K ~ |dx_n| / |dx_{n-1}|^2, so
 // the step AFTER the one just taken would be ~ |dx_n|^3 / |dx_{n-1}|^2; once that is below 1e-13 |r| (three orders
-// inside the 1e-10 position bar) the root is converged and the confirming evaluation is skipped.  From the third iteration on the residual is also compared
-// with the rounding floor of its own evaluation (ill-conditioned roots next to a caustic stall there).
-// Verification: all five converged and distinct (Vieta: sum of roots = -c4/c5).
-// Recovery (at most once per solve): when two chains ran into the same root, or up to two chains have not
-// converged after TWK_RECOVER_AT (4) sweeps, the three or four good distinct roots fix the others through Vieta's formulas
-// (sum of roots = -c4/c5, product = -c0/c5: one missing root directly, two as the roots of a quadratic); these
-// are polished by the same Newton sweeps and the verification is repeated.
+// inside the 1e-10 position bar) the root is converged and the confirming evaluation is skipped.  The rule compares
+// orders of magnitude and runs on integer magnitude keys (mag_key).  From the third sweep on the residual is also
+// compared with the rounding floor of its own evaluation (ill-conditioned roots next to a caustic stall there).
+// Verification: the product of the five roots = -c0 (relative 1e-9; catches two chains on one root), and, once all
+// five are iterated, their sum = -c4.
+// Recovery (at most once per solve): when the product does not verify, or a chain has not converged after
+// TWK_RECOVER_AT sweeps, chain 4 is iterated like the others for three sweeps; then the three or four good distinct roots
+// fix the others through Vieta's formulas (sum = -c4, product = -c0: one missing root directly, two as the roots of a
+// quadratic -- which is also the fast way through a nearly double root, where Newton converges only linearly); these are
+// polished by the same Newton sweeps and verified again.
 // Returns 0 when that fails too; the caller then falls back to the cold solver quintic_roots().
 // r[] holds the seeds on entry and the roots on exit.
 // Two converged chains are the same root when they agree to 1e-6 of their size (RELATIVE: next to a planet of
@@ -341,10 +345,24 @@ TWK_NOINLINE SeededState seeded_recover(cd c0, cd c5, cd tot, SeededState S) {
   return S;
 }
 
-// One Newton step of root x on the quintic c.  kFloor: also compare the residual with the rounding floor of its own
-// evaluation.  Returns true when the root is converged (see the stop rule above); prev = |dx| of the previous step.
+// One Newton step of root x on the monic quintic c.  kFloor: also compare the residual with the rounding floor of its
+// own evaluation.  Returns true when the root is converged (see the stop rule above); prev = key of the previous |dx|.
+// Magnitude key of a complex number: 2^16 (log2 max(|Re|, |Im|) + 1023), piecewise linear in the mantissa -- the high
+// word of the larger component.  The stop rule compares orders of magnitude; it runs on these keys in the integer ALU
+// instead of spending FP64 multiplications on it.  NaN gives the largest key (never "converged"), zero gives 0.
+TWK_HD int mag_key(cd v) {
+#ifdef __CUDA_ARCH__
+  return max(__double2hiint(v.x) & 0x7fffffff, __double2hiint(v.y) & 0x7fffffff) >> 4;
+#else
+  return 0;
+#endif
+}
+constexpr int kKeyOne = 1023 << 16;                  // key of 1.0
+constexpr int kKeyStop = (0x3d3c2000 >> 4) - kKeyOne;   // 2^16 log2(TWK_STOP_FACTOR * eps) = 2^16 log2(1e-13)
+constexpr int kKeyMargin = 1 << 16;                  // |dx| <= 2 max-norm(dx) and the piecewise-linear log: a factor 2 on |dx|^3
+
 template <bool kFloor>
-TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev, bool check = true) {
+TWK_HD bool newton_step(const cd (&c)[6], cd& x, int& prev, bool check = true) {
   TWK_COUNT(newton_eval);
   // c[0..4] are the coefficients of the MONIC quintic (c[5] is not read): the first two Horner steps are additions
   cd p = mk(x.x + c[4].x, x.y + c[4].y);
@@ -367,21 +385,19 @@ TWK_HD bool newton_step(const cd (&c)[6], cd& x, double& prev, bool check = true
   const double inv = slope ? rcp1(dn) : 0.0;
   const cd dx = mk(fma(p.x, d.x, p.y * d.y) * inv, fma(p.y, d.x, -(p.x * d.y)) * inv);
   x = x - dx;
-  const double sdx = abs1(dx);
+  // stop rule: |dx|^3 <= 1e-13 |x| |dx_prev|^2, on magnitude keys (prev = key of the previous step, 0 before the first)
+  const int ks = mag_key(dx);
   bool conv = false;
-  if (check) {   // (the first sweep of a solve has no previous step: only a later one can satisfy the rule)
-    const double ar = abs1(x);
-    conv = slope && (sdx * sdx * sdx <= (TWK_STOP_FACTOR * kEps) * ar * prev * prev || sdx <= kEps * ar);
-  }
-  prev = sdx;
+  if (check) conv = slope && (3 * ks + kKeyMargin <= kKeyStop + mag_key(x) + 2 * prev);
+  prev = ks;
   return conv;
 }
 
 // Returns 0 = failed (use the cold solver), 1 = solved, 2 = solved after the Vieta recovery.
 TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product) {
-  double prev[5];
+  int prev[5];
 #pragma unroll
-  for (int k = 0; k < 5; ++k) prev[k] = 0.0;
+  for (int k = 0; k < 5; ++k) prev[k] = 0;
   const cd tot = -c[4];               // sum of the five roots (monic coefficients)
   unsigned done = 0;
   // sweeps 0 and 1: every root needs them (the stop rule wants two steps), so all five chains run unconditionally
@@ -441,7 +457,7 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
       for (int k = 0; k < 5; ++k)
         if (!(S.done >> k & 1u)) {
           r[k] = S.r[k];
-          prev[k] = 0.0;
+          prev[k] = 0;
         }
       done = S.done;
     }
@@ -451,7 +467,7 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
     for (int k = 0; k < 5; ++k) {
       if (done & (1u << k)) continue;
       cd x = r[0];
-      double pv = prev[0];
+      int pv = prev[0];
 #pragma unroll
       for (int j = 1; j < 5; ++j)
         if (j == k) { x = r[j]; pv = prev[j]; }

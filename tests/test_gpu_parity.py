@@ -222,7 +222,7 @@ def test_full_size_config3_sampled_outputs(ctx):
     idx = np.sort(np.random.default_rng(5).choice(wl.n_sources, 3000, replace=False))
     ref = api.magnify(wl.subset(idx), 1e-6, mode=1, prec=0)
     rel = np.abs(g["mu"][idx] / ref["mu"] - 1)
-    assert rel.max() < 3e-4, rel.max()         # outputs at tol 1e-4 vs converged reference: few x tol
+    assert rel.max() <= 1e-4, rel.max()        # outputs at tol 1e-4 vs the converged reference: within the tolerance
     assert np.median(rel) < 1e-5
 
 
