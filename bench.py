@@ -404,8 +404,12 @@ def main():
                 t = stage_ms.get(k, 0.0)
                 if t > 0 and c["flop"] > 0:
                     a = c["flop"] / (t * 1e-3) / 1e12
+                    inst = c["dfma"] + c["dmul"] + c["dadd"]
                     o[k] = {"achieved_tflops": a, "frac": a / peak_tf, "flop": c["flop"], "dram_bytes": c["dram_bytes"],
-                            "fp64_pipe_pct_ncu": c["fp64_pipe_pct"]}
+                            "fp64_pipe_pct_ncu": c["fp64_pipe_pct"], "issue_active_pct_ncu": c["issue_active_pct"],
+                            # what `frac` would read with the FP64 pipe busy every cycle, given this kernel's share of
+                            # DFMA (2 flop) among its FP64 instructions
+                            "mix_limit": c["flop"] / (2.0 * inst) if inst > 0 else None}
             return o
 
         sm = R["stage_ms"]
@@ -443,6 +447,8 @@ def main():
                          "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x "
                                         f"{sm_max_mhz:.0f} MHz (MEASURED_PEAKS.json has no FP64 figure)",
                          "peak_probe_tflops": probe_tf, "frac_of_probe": (dom["achieved_tflops"] / probe_tf) if dom else None,
+                         "mix_limit": dom["mix_limit"] if dom else None,
+                         "fp64_pipe_active_pct_ncu": dom["fp64_pipe_pct_ncu"] if dom else None,
                          "flop_per_point": (dom["flop"] / (64.0 * n)) if dom else None, "points_per_launch": 64 * n,
                          "kernel_ms": sm, "stage1_share_of_step": s1 / (ms / args.steps),
                          "per_stage": fr,
