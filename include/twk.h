@@ -120,6 +120,19 @@ int twk_magnify_lightcurve(twk_ctx* ctx, size_t n_models, const double* s, const
                            const int32_t* model_id, const double* t, double rel_tol, double* out_mu, double* out_err,
                            int32_t* out_nsamples, uint32_t* out_status, void* stream);
 
+/* Light-curve front end with lens ORBITAL MOTION (contour integration is "particularly suitable
+ * for modeling lens orbital motion" because every epoch may have its own lens -- nothing is precomputed per lens).  As
+ * twk_magnify_lightcurve, with the lens of each epoch moved to first order in time (the paper gives no parametrisation;
+ * this is the usual two-rate one):
+ *     s(t) = s + ds_dt (t - t0),      alpha(t) = alpha + dalpha_dt (t - t0),
+ * q, rho, u0, tE unchanged.  An epoch whose s(t) leaves (0, inf) gives NaN with TWK_ST_DOMAIN, like any invalid parameter.
+ *   ds_dt, dalpha_dt    DEVICE double[n_models]   rates per unit of t (required; zeros reproduce twk_magnify_lightcurve) */
+int twk_magnify_lightcurve_orbital(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                                   const double* t0, const double* u0, const double* tE, const double* alpha,
+                                   const double* ds_dt, const double* dalpha_dt, size_t n_sources, const int32_t* model_id,
+                                   const double* t, double rel_tol, double* out_mu, double* out_err, int32_t* out_nsamples,
+                                   uint32_t* out_status, void* stream);
+
 /* Fixed-sampling mode (BASELINE config 1 and the parity harness): theta_j = 2 pi j / N, no adaptivity.
  *   out_z       DEVICE double[n_sources][N][5][2]  optional: all five roots, CM frame, order unspecified
  *   out_kind    DEVICE int8[n_sources][N][5]       optional: 0 ghost, +1 / -1 real image of that parity

@@ -17,7 +17,7 @@ _lib = None
 
 TWK_ST_CONVERGED, TWK_ST_CAP, TWK_ST_REPAIRED, TWK_ST_DOMAIN, TWK_ST_NUMERIC, TWK_ST_SLOPE, TWK_ST_POINT = 1, 2, 4, 8, 16, 32, 64
 
-SYMBOLS = ["twk_default_options", "twk_create", "twk_destroy", "twk_workspace_bytes", "twk_magnify", "twk_magnify_lightcurve",
+SYMBOLS = ["twk_default_options", "twk_create", "twk_destroy", "twk_workspace_bytes", "twk_magnify", "twk_magnify_lightcurve", "twk_magnify_lightcurve_orbital",
            "twk_images_fixed", "twk_images_fixed_seeded", "twk_stage1_records",
            "twk_magnify_host", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_debug_counters", "twk_strerror", "twk_version"]
 
@@ -52,6 +52,7 @@ def lib():
         L.twk_workspace_bytes.restype = sz
         L.twk_magnify.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
         L.twk_magnify_lightcurve.argtypes = [vp, sz, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
+        L.twk_magnify_lightcurve_orbital.argtypes = [vp, sz, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
         L.twk_magnify_host.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
         L.twk_images_fixed.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, vp]
         L.twk_images_fixed_seeded.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
@@ -181,6 +182,23 @@ class Context:
         _check(lib().twk_magnify_lightcurve(self._h, int(s.shape[0]), _ptr(s), _ptr(q), _ptr(rho), _ptr(t0), _ptr(u0), _ptr(tE),
                                             _ptr(alpha), n, _ptr(model_id), _ptr(t), float(rel_tol), _ptr(mu), _ptr(err),
                                             _ptr(ns), _ptr(st), _stream_ptr(stream)), "twk_magnify_lightcurve")
+        return dict(mu=mu, err=err, nsamples=ns, status=st)
+
+    def twk_magnify_lightcurve_orbital(self, s, q, rho, t0, u0, tE, alpha, ds_dt, dalpha_dt, t, model_id=None, rel_tol=1e-4,
+                                       stream=None):
+        """Light-curve front end with first-order lens orbital motion: as twk_magnify_lightcurve plus the per-model rates
+        ds_dt, dalpha_dt (float64 CUDA [n_models]); every epoch gets its own lens on the device."""
+        import torch
+        n = int(t.shape[0])
+        dev = t.device
+        mu = torch.empty(n, dtype=torch.float64, device=dev)
+        err = torch.empty(n, dtype=torch.float64, device=dev)
+        ns = torch.empty(n, dtype=torch.int32, device=dev)
+        st = torch.empty(n, dtype=torch.int32, device=dev)
+        _check(lib().twk_magnify_lightcurve_orbital(self._h, int(s.shape[0]), _ptr(s), _ptr(q), _ptr(rho), _ptr(t0), _ptr(u0),
+                                                    _ptr(tE), _ptr(alpha), _ptr(ds_dt), _ptr(dalpha_dt), n, _ptr(model_id),
+                                                    _ptr(t), float(rel_tol), _ptr(mu), _ptr(err), _ptr(ns), _ptr(st),
+                                                    _stream_ptr(stream)), "twk_magnify_lightcurve_orbital")
         return dict(mu=mu, err=err, nsamples=ns, status=st)
 
     def twk_images_fixed(self, s, q, rho, zeta, N, model_id=None, want_z=True, want_kind=True, stream=None):

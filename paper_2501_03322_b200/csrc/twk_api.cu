@@ -227,7 +227,7 @@ int twk_magnify(twk_ctx* ctx, size_t n_models, const double* s, const double* q,
   if (n_sources == 0) return TWK_OK;
   if (!out_mu || !(rel_tol > 0.0)) return TWK_EINVAL;
   const twk::Batch b{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame,
-                     nullptr, nullptr, nullptr, nullptr, nullptr};
+                     nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   return magnify_impl(ctx, b, rel_tol, out_mu, out_err, out_nsamples, out_status, stream_);
 }
 
@@ -240,7 +240,21 @@ int twk_magnify_lightcurve(twk_ctx* ctx, size_t n_models, const double* s, const
   if (n_sources == 0) return TWK_OK;
   if (!t0 || !u0 || !tE || !alpha || !out_mu || !(rel_tol > 0.0)) return TWK_EINVAL;
   const twk::Batch b{s, q, rho, model_id, nullptr, (long long)n_models, (long long)n_sources, ctx->opt.frame,
-                     t, t0, u0, tE, alpha};
+                     t, t0, u0, tE, alpha, nullptr, nullptr};
+  return magnify_impl(ctx, b, rel_tol, out_mu, out_err, out_nsamples, out_status, stream_);
+}
+
+int twk_magnify_lightcurve_orbital(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
+                                   const double* t0, const double* u0, const double* tE, const double* alpha,
+                                   const double* ds_dt, const double* dalpha_dt, size_t n_sources, const int32_t* model_id,
+                                   const double* t, double rel_tol, double* out_mu, double* out_err, int32_t* out_nsamples,
+                                   uint32_t* out_status, void* stream_) {
+  const int rc = check_batch(ctx, n_models, s, q, rho, n_sources, model_id, t);
+  if (rc != TWK_OK) return rc;
+  if (n_sources == 0) return TWK_OK;
+  if (!t0 || !u0 || !tE || !alpha || !ds_dt || !dalpha_dt || !out_mu || !(rel_tol > 0.0)) return TWK_EINVAL;
+  const twk::Batch b{s, q, rho, model_id, nullptr, (long long)n_models, (long long)n_sources, ctx->opt.frame,
+                     t, t0, u0, tE, alpha, ds_dt, dalpha_dt};
   return magnify_impl(ctx, b, rel_tol, out_mu, out_err, out_nsamples, out_status, stream_);
 }
 

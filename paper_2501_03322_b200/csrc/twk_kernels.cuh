@@ -68,6 +68,10 @@ struct Batch {
   const double* u0;          // [n_models]
   const double* tE;          // [n_models]
   const double* alpha;       // [n_models]
+  // lens orbital motion to first order (twk_magnify_lightcurve_orbital): s(t) = s + ds_dt (t - t0),
+  // alpha(t) = alpha + dalpha_dt (t - t0); null = static lens
+  const double* ds_dt;       // [n_models] or null
+  const double* dalpha_dt;   // [n_models] or null
 };
 
 struct SourceParams {
@@ -82,11 +86,18 @@ __device__ __forceinline__ SourceParams load_source(const Batch& b, long long sr
   SourceParams P;
   const long long m_in = b.model_id ? (long long)b.model_id[src] : (b.n_models == 1 ? 0 : src);
   const long long m = (m_in >= 0 && m_in < b.n_models) ? m_in : 0;   // never read outside the model arrays
-  const double s = b.s[m], q = b.q[m], rho = b.rho[m];
+  double s = b.s[m];
+  const double q = b.q[m], rho = b.rho[m];
   if (b.t) {
-    const double tau = (b.t[src] - b.t0[m]) / b.tE[m], u0 = b.u0[m];
+    const double dt = b.t[src] - b.t0[m];
+    const double tau = dt / b.tE[m], u0 = b.u0[m];
+    double alpha = b.alpha[m];
+    if (b.ds_dt) {   // the lens of THIS epoch (what contour integration is preferred for)
+      s = fma(b.ds_dt[m], dt, s);
+      alpha = fma(b.dalpha_dt[m], dt, alpha);
+    }
     double sa, ca;
-    sincos(b.alpha[m], &sa, &ca);
+    sincos(alpha, &sa, &ca);
     P.zc = mk(-(tau * ca - u0 * sa), -(tau * sa + u0 * ca));
   } else {
     P.zc = mk(b.zeta[2 * src], b.zeta[2 * src + 1]);
