@@ -91,6 +91,13 @@ int cuda_fail(cudaError_t e) {
 // teams per CTA kept in step by CTA-wide barriers: 1 x 6 CTAs/SM 36.5 ms, 2 x 3: 36.0, 3 x 2: 38.3, 4 x 1: 47.8,
 // 6 x 1: 43.7 -- coupling the teams costs more than the shared instruction stream saves, so one team per CTA it is.
 void launch_stage1(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t stream) {
+  {   // powers of the first iteration's interval width (twk::link_const on the host)
+    const double dth = twk::kTwoPi / double(twk::kThreads), dth2 = dth * dth, dth3 = dth2 * dth;
+    a.K1.dth2 = dth2;
+    a.K1.c24 = dth3 * (1.0 / 24.0);
+    a.K1.c12 = dth * (1.0 / 12.0);
+    a.K1.c48 = dth3 * (1.0 / 48.0);
+  }
   const size_t smem = twk::stage1_smem_bytes();   // below the 48 KB default limit: no opt-in needed
   static_assert(twk::stage1_smem_bytes() <= 48 * 1024, "stage-1 shared memory needs the opt-in attribute");
   // groups of up to 64 sources per CTA pass; a small batch takes smaller groups so that every resident CTA gets work

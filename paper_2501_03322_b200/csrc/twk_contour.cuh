@@ -149,7 +149,10 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     Res[k] = mk(y.x - eta[k].x - f.x, y.y - eta[k].y + f.y);   // Eq.(12): y - eta - conj(f)
     J[k] = 1.0 - norm2(fp[k]);                           // Eq.(7)
     R2[k] = norm2(Res[k]);
-    finite = finite && isfinite(R2[k]) && isfinite(J[k]);
+  }
+  {   // all ten finite?  |R|^2 >= 0 and J <= 1: their sums cannot cancel an infinity and NaN propagates
+    const double sr = ((R2[0] + R2[1]) + (R2[2] + R2[3])) + R2[4], sj = ((J[0] + J[1]) + (J[2] + J[3])) + J[4];
+    finite = isfinite(sr) && isfinite(sj);
   }
   // a5: residual detector, 2-cycle reading (G-1): the two largest-|R| roots (ia, ib) are a ghost pair iff
   // R_ia = eta_ib - eta_ia and R_ib = eta_ia - eta_ib ("a pair of ghost images with opposite residuals").
@@ -165,20 +168,24 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
       scr.at(10 + k) = Res[k].x;
       scr.at(15 + k) = Res[k].y;
     }
+    // the two largest |R|^2 by integer maxima over keys (high word of the non-negative double, index in the low three
+    // bits): |R|^2 of a ghost is orders of magnitude above the rounding residue of a real image, 2^-17 relative resolves
+    // every case that matters; among real images (or between the two ghosts, whose |R| are equal) any order will do
+    unsigned key[5];
 #pragma unroll
-    for (int k = 1; k < 5; ++k) {
-      if (R2[k] > mA) {
-        mB = mA; ib = ia;
-        mA = R2[k]; ia = k;
-      } else if (R2[k] > mB) {
-        mB = R2[k]; ib = k;
-      }
-    }
-    const int jb = ib < 0 ? 0 : ib;   // (only when every |R| is NaN)
+    for (int k = 0; k < 5; ++k) key[k] = ((unsigned)__double2hiint(R2[k]) & ~7u) | (unsigned)k;
+    const unsigned t1 = max(key[0], key[1]), s1 = min(key[0], key[1]), t2 = max(key[2], key[3]), s2 = min(key[2], key[3]);
+    const unsigned T4 = max(t1, t2), U4 = max(min(t1, t2), max(s1, s2));   // first and second of the first four
+    const unsigned T5 = max(T4, key[4]), U5 = max(min(T4, key[4]), U4);
+    ia = (int)(T5 & 7u);
+    const int jb = (int)(U5 & 7u);
+    ib = jb;
     eA = mk(scr.at(ia), scr.at(5 + ia));
     rA = mk(scr.at(10 + ia), scr.at(15 + ia));
     eB = mk(scr.at(jb), scr.at(5 + jb));
     rB = mk(scr.at(10 + jb), scr.at(15 + jb));
+    mA = norm2(rA);   // (= R2[ia], R2[ib] bit for bit)
+    mB = norm2(rB);
   } else {
 #pragma unroll
     for (int k = 1; k < 5; ++k) {
@@ -192,41 +199,43 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   }
   const cd dab = eB - eA;
   const bool ghost = norm2(rA - dab) < mA && norm2(rB + dab) < mB;
-  int kind[5];
-  int nreal = 0, npos = 0;
+  // kinds as bit masks over the five roots: gmask = ghost pair, posm / negm = real images of positive / negative parity
+  // (Eq.(7): p = sign J)
+  const unsigned gmask = ghost ? ((1u << ia) | (1u << (ib & 7))) : 0u;
+  unsigned jpos = 0;
 #pragma unroll
-  for (int k = 0; k < 5; ++k) {
-    const bool g = ghost && (k == ia || k == ib);
-    kind[k] = g ? 0 : (J[k] > 0.0 ? 1 : -1);             // Eq.(7)
-    nreal += !g;
-    npos += (kind[k] > 0);
-  }
+  for (int k = 0; k < 5; ++k) jpos |= (J[k] > 0.0) ? (1u << k) : 0u;
+  unsigned posm = jpos & ~gmask, negm = ~jpos & ~gmask & 31u;
+  const int nreal = 5 - __popc(gmask);
+  int npos = __popc(posm);
   // parity sum must be -1.  Repair by flipping the smallest-|J| image of the over-represented parity.
   flags |= finite ? 0 : kPointNonFinite;
   const int want = (nreal - 1) >> 1;
   for (int guard = 0; guard < 5 && npos != want; ++guard) {
-    const int over = (npos > want) ? 1 : -1;
+    const bool over = npos > want;
+    const unsigned cand = over ? posm : negm;
     int best = -1;
     double bj = 1e300;
 #pragma unroll
     for (int k = 0; k < 5; ++k)
-      if (kind[k] == over && fabs(J[k]) < bj) { bj = fabs(J[k]); best = k; }
-#pragma unroll
-    for (int k = 0; k < 5; ++k)
-      if (k == best) kind[k] = -over;
-    npos -= over;
+      if ((cand >> k & 1u) && fabs(J[k]) < bj) { bj = fabs(J[k]); best = k; }
+    if (best >= 0) {
+      posm ^= 1u << best;
+      negm ^= 1u << best;
+    }
+    npos += over ? -1 : 1;
     flags |= kPointRepaired;
   }
-  // record: positives to slots 0.., negatives to slots 2..
-  int sp = 0, sm = 2;
+  // record: positives to slots 0.., negatives to slots 2..: the slot of a root is the number of same-parity roots before it
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
     const cd z = mk(eta[k].x + L.z2, eta[k].y);
+    const bool isp = posm >> k & 1u, isn = negm >> k & 1u;
     if (out_z) { out_z[2 * k] = z.x; out_z[2 * k + 1] = z.y; }
-    if (out_kind) out_kind[k] = (int8_t)kind[k];
-    // (slots stay inside the record whatever the kinds are: with non-finite J every kind is -1)
-    if (kind[k] != 0 && (kind[k] > 0 ? sp < 2 : sm < 5)) {
-      const int slot = (kind[k] > 0) ? sp++ : sm++;
+    if (out_kind) out_kind[k] = (int8_t)(isp ? 1 : (isn ? -1 : 0));
+    const int slot = isp ? __popc(posm & ((1u << k) - 1u)) : 2 + __popc(negm & ((1u << k) - 1u));
+    // (slots stay inside the record whatever the kinds are: with non-finite J every root counts as negative)
+    if ((isp || isn) && slot < (isp ? 2 : 5)) {
       const double invJ = rcp(J[k]);
       // z' = (zeta' - conj(f') conj(zeta')) / J                       Eq.(10), repaired (E-2)
       const cd t = conj(fp[k]) * conj(dzeta);
@@ -509,7 +518,8 @@ TWK_HD int crossed_is_shorter(double s00, double s11, double s01, double s10) {
   return (sqrt(s01) + sqrt(s10)) < (sqrt(s00) + sqrt(s11));
 }
 
-TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth, double slope_gate2, double slope_cos2) {
+// K = link_const(dth) of the interval's width dth = theta_B - theta_A > 0
+TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, const LinkConst& K, double slope_gate2, double slope_cos2) {
   Piece P;
   P.dA = 0.0;
   P.err = 0.0;
@@ -588,7 +598,6 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth, double 
     }
   }
   // ---- a7: area and error of every link (one copy of the code; 3 or 4 or 5 trips) ----------------------------
-  const LinkConst K = link_const(dth);
 #pragma unroll 1
   for (int l = 0; l < nl; ++l) {
     const int ka = (int)(links & 15u), kb = (int)((links >> 4) & 15u);
@@ -629,10 +638,13 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth, double 
     P.crossing = creation ? 1 : -1;
     P.dA += chord + dAp;
     const double E1 = fabs(wpl + wmi) * dtt3 * (1.0 / 48.0);            // Eq.(18)
-    const double E3 = 0.1 * fabs(dAp) * dth * dth;
+    const double E3 = 0.1 * fabs(dAp) * K.dth2;
     P.err += E1 + E2 + E3;
   }
   return P;
+}
+TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, double dth, double slope_gate2, double slope_cos2) {
+  return eval_interval(A, B, link_const(dth), slope_gate2, slope_cos2);
 }
 
 // ------------------------------------------------------------------------------------------------------------

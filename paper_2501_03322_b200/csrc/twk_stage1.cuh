@@ -39,6 +39,8 @@ struct Stage1Args {
   double tol;
   double slope_gate2;    // square of the slope detector's proximity gate (twk_options.slope_gate)
   double slope_cos2;     // square of the largest |cos| still counted as perpendicular (twk_options.slope_cos)
+  LinkConst K1;          // powers of the first iteration's interval width 2 pi / 64 (kernel parameters are constant-bank
+                         // operands: no instruction materialises them)
   int ps_test;           // N1: point-source adequacy tests in front of the contour path (twk_options.point_source_test)
   int guard;             // L-4 guard: hidden-crossing term in the interval estimates (twk_options.hidden_crossing_guard)
   int group;             // sources per group, 1..64 (smaller for small batches: more CTAs get work)
@@ -172,7 +174,7 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
       double A, E;
       constexpr int kSlopeVote = 1 << 8;
       for (;;) {
-        P = eval_interval(mine, next, kTwoPi / double(kThreads), p.slope_gate2, p.slope_cos2);
+        P = eval_interval(mine, next, p.K1, p.slope_gate2, p.slope_cos2);
         if (kGuard && P.crossing == 0) {
           const double h = kTwoPi / double(kThreads);
           P.err += hidden_crossing_term(RecRef{recs + ((t + kThreads - 1) & (kThreads - 1)), kThreads}, mine, next,
