@@ -108,10 +108,10 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
       const double ex = seeds[k * seed_stride], ey = seeds[(5 + k) * seed_stride];
-      const double ax = seeds[(10 + k) * seed_stride], ay = seeds[(15 + k) * seed_stride];
-      const double bx = seeds[(20 + k) * seed_stride], by = seeds[(25 + k) * seed_stride];
-      // A delta + B conj(delta)
-      eta[k] = mk(ex + fma(ax + bx, dx, (by - ay) * dy), ey + fma(ay + by, dx, (ax - bx) * dy));
+      const double pxx = seeds[(10 + k) * seed_stride], pxy = seeds[(15 + k) * seed_stride];
+      const double pyx = seeds[(20 + k) * seed_stride], pyy = seeds[(25 + k) * seed_stride];
+      // eta + A delta + B conj(delta) as a real 2 x 2 map of (Re delta, Im delta), prepared by centre_seeds()
+      eta[k] = mk(fma(pxx, dx, fma(pxy, dy, ex)), fma(pyx, dx, fma(pyy, dy, ey)));
     }
     {   // the seeded solve works on the monic quintic; the cold solver below gets the same coefficients with c5 = 1
       const cd i5 = crecip(c[5]);
@@ -139,8 +139,12 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   bool finite = true;
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
-    const cd a = crecip(mk(-L.s - eta[k].x, -eta[k].y));
-    const cd b = crecip(-eta[k]);
+    // a = 1 / (z1 - z), b = 1 / (z2 - z): ONE reciprocal for both, 1 / (|z1 - z|^2 |z2 - z|^2)
+    const cd za = mk(-L.s - eta[k].x, -eta[k].y), zb = -eta[k];
+    const double na = norm2(za), nb = norm2(zb);
+    const double rab = rcp(na * nb);
+    const double ia_ = rab * nb, ib_ = rab * na;
+    const cd a = mk(za.x * ia_, -za.y * ia_), b = mk(zb.x * ib_, -zb.y * ib_);
     const cd a2 = a * a, b2 = b * b;
     const cd f = L.m1 * a + L.m2 * b;                    // Eq.(7)
     fp[k] = L.m1 * a2 + L.m2 * b2;
@@ -236,7 +240,7 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     const int slot = isp ? __popc(posm & ((1u << k) - 1u)) : 2 + __popc(negm & ((1u << k) - 1u));
     // (slots stay inside the record whatever the kinds are: with non-finite J every root counts as negative)
     if ((isp || isn) && slot < (isp ? 2 : 5)) {
-      const double invJ = rcp(J[k]);
+      const double invJ = rcp1(J[k]);   // (40 bits: z' and z'^z'' only enter the parabolic corrections and the estimates)
       // z' = (zeta' - conj(f') conj(zeta')) / J                       Eq.(10), repaired (E-2)
       const cd t = conj(fp[k]) * conj(dzeta);
       const cd zp = mk((dzeta.x - t.x) * invJ, (dzeta.y - t.y) * invJ);
@@ -278,9 +282,10 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
 
 // Seed block of one source (kSeedDoubles doubles, element e at seeds[e * stride]):
 //   [0..4] Re eta_k, [5..9] Im eta_k   the five planet-frame roots of the point source at the source CENTRE (cold solve)
-//   [10..14] Re A_k, [15..19] Im A_k, [20..24] Re B_k, [25..29] Im B_k
-//                                      first-order response of root k to a displacement delta of the source:
-//                                      d eta_k = A_k delta + B_k conj(delta)
+//   [10..14] Re(A_k + B_k), [15..19] Im(B_k - A_k), [20..24] Im(A_k + B_k), [25..29] Re(A_k - B_k)
+//                                      first-order response of root k to a displacement delta of the source,
+//                                      d eta_k = A_k delta + B_k conj(delta), stored as the real 2 x 2 map of
+//                                      (Re delta, Im delta) -> (Re d eta_k, Im d eta_k): four FMAs per root and sample
 //   [30]                               1 when two roots are closer than 1e-6 of the roots' scale (next to a planet of
 //                                      tiny q): the seeded solve then also verifies the PRODUCT of the roots
 // The quintic's roots are the fixed points (real images) and the 2-cycle (ghost pair) of T(z) = zeta - conj f(z)
@@ -349,10 +354,11 @@ TWK_HD void centre_seeds(const Lens& L, cd zc, double rho, double* seeds, int st
     dmin2_all = fmin(dmin2_all, dmin2);
     seeds[k * st] = eta[k].x;
     seeds[(5 + k) * st] = eta[k].y;
-    seeds[(10 + k) * st] = A.x;
-    seeds[(15 + k) * st] = A.y;
-    seeds[(20 + k) * st] = B.x;
-    seeds[(25 + k) * st] = B.y;
+    // A delta + B conj(delta) = (A.x + B.x) dx + (B.y - A.y) dy + i [(A.y + B.y) dx + (A.x - B.x) dy]
+    seeds[(10 + k) * st] = A.x + B.x;
+    seeds[(15 + k) * st] = B.y - A.y;
+    seeds[(20 + k) * st] = A.y + B.y;
+    seeds[(25 + k) * st] = A.x - B.x;
   }
   const double scale = abs1(eta[0]) + abs1(eta[1]) + abs1(eta[2]) + abs1(eta[3]) + abs1(eta[4]);
   seeds[30 * st] = (dmin2_all < 1e-12 * scale * scale) ? 1.0 : 0.0;
@@ -509,12 +515,14 @@ TWK_HD void link_terms(const RecRef& A, const RecRef& B, int ka, int kb, double 
 }
 
 // 2 x 2 minimum-total-distance matching from SQUARED distances: returns 1 when the crossed pairing (0-1, 1-0) is
-// shorter than the straight one (0-0, 1-1); ties keep the straight pairing (reading L-3).  When one pairing has
-// both distances below half of both distances of the other, 2 max < min settles the comparison of the sums without
-// square roots (the decision is the same as the exact one whenever the shortcut applies).
+// shorter than the straight one (0-0, 1-1); ties keep the straight pairing (reading L-3).  Short cut without square
+// roots: 2 (s00 + s11) < min(s01, s10) gives sqrt s00 + sqrt s11 <= sqrt(2 (s00 + s11)) < sqrt(min) <= sqrt s01 + sqrt s10,
+// so the straight pairing is the shorter one (and the mirror statement); the decision is the exact one whenever the
+// short cut applies, and it applies unless the images are about as close to each other as to their successors.
 TWK_HD int crossed_is_shorter(double s00, double s11, double s01, double s10) {
-  if (4.0 * fmax(s00, s11) < fmin(s01, s10)) return 0;
-  if (4.0 * fmax(s01, s10) < fmin(s00, s11)) return 1;
+  const double st = 2.0 * (s00 + s11), cr = 2.0 * (s01 + s10);
+  if (st < s01 && st < s10) return 0;
+  if (cr < s00 && cr < s11) return 1;
   return (sqrt(s01) + sqrt(s10)) < (sqrt(s00) + sqrt(s11));
 }
 

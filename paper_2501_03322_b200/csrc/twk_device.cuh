@@ -345,50 +345,58 @@ TWK_NOINLINE SeededState seeded_recover(cd c0, cd c5, cd tot, SeededState S) {
   return S;
 }
 
-// One Newton step of root x on the monic quintic c.  kFloor: also compare the residual with the rounding floor of its
-// own evaluation.  Returns true when the root is converged (see the stop rule above); prev = key of the previous |dx|.
-// Magnitude key of a complex number: 2^16 (log2 max(|Re|, |Im|) + 1023), piecewise linear in the mantissa -- the high
-// word of the larger component.  The stop rule compares orders of magnitude; it runs on these keys in the integer ALU
-// instead of spending FP64 multiplications on it.  NaN gives the largest key (never "converged"), zero gives 0.
+// Magnitude key of a complex number: 2^16 (log2(|Re| + |Im|) + 1023), piecewise linear in the mantissa -- the high
+// word of the 1-norm.  The stop rule compares orders of magnitude; it runs on these keys in the integer ALU instead of
+// spending FP64 multiplications on it.  NaN gives the largest key (never "converged"), zero gives 0.
 TWK_HD int mag_key(cd v) {
 #ifdef __CUDA_ARCH__
-  return max(__double2hiint(v.x) & 0x7fffffff, __double2hiint(v.y) & 0x7fffffff) >> 4;
+  return (__double2hiint(abs1(v)) & 0x7fffffff) >> 4;
 #else
   return 0;
 #endif
 }
 constexpr int kKeyOne = 1023 << 16;                  // key of 1.0
 constexpr int kKeyStop = (0x3d3c2000 >> 4) - kKeyOne;   // 2^16 log2(TWK_STOP_FACTOR * eps) = 2^16 log2(1e-13)
-constexpr int kKeyMargin = 1 << 16;                  // |dx| <= 2 max-norm(dx) and the piecewise-linear log: a factor 2 on |dx|^3
+constexpr int kKeyMargin = 1 << 16;                  // the piecewise-linear log2 (< 0.09 per key): a factor 2 on |dx|^3 covers it
 
-template <bool kFloor>
-TWK_HD bool newton_step(const cd (&c)[6], cd& x, int& prev, bool check = true) {
-  TWK_COUNT(newton_eval);
-  // c[0..4] are the coefficients of the MONIC quintic (c[5] is not read): the first two Horner steps are additions
-  cd p = mk(x.x + c[4].x, x.y + c[4].y);
-  cd d = mk(x.x + p.x, x.y + p.y);
+// Horner for p and p' of the MONIC quintic (c[5] is not read): the first two steps are additions
+TWK_HD void horner_pd(const cd (&c)[6], cd x, cd& p, cd& d) {
+  p = mk(x.x + c[4].x, x.y + c[4].y);
+  d = mk(x.x + p.x, x.y + p.y);
   p = cfma(p, x, c[3]);
 #pragma unroll
   for (int i = 2; i >= 0; --i) {
     d = cfma(d, x, p);
     p = cfma(p, x, c[i]);
   }
-  if (kFloor) {
+}
+// One Newton step x <- x - p / p'; returns the magnitude key of the step.  p' = 0 needs no branch: the reciprocal of 0
+// is an infinity whose refinement is NaN, the root becomes NaN, its key the largest there is, and a chain that never
+// "converges" is what the Vieta recovery replaces.
+TWK_HD int newton_move(cd p, cd d, cd& x) {
+  const double inv = rcp1(norm2(d));
+  const cd dx = mk(fma(p.x, d.x, p.y * d.y) * inv, fma(p.y, d.x, -(p.x * d.y)) * inv);
+  x = x - dx;
+  return mag_key(dx);
+}
+// stop rule: |dx|^3 <= 1e-13 |x| |dx_prev|^2 on magnitude keys (kprev = 0: no previous step, only dx = 0 passes)
+TWK_HD bool newton_converged(int ks, int kprev, cd x) { return 3 * ks + kKeyMargin <= kKeyStop + mag_key(x) + 2 * kprev; }
+
+// The step of the later sweeps (one root at a time): also compares the residual with the rounding floor of its own
+// evaluation.  Returns true when the root is converged; prev = key of the previous |dx|.
+TWK_HD bool newton_step_floor(const cd (&c)[6], cd& x, int& prev) {
+  TWK_COUNT(newton_eval);
+  cd p, d;
+  horner_pd(c, x, p, d);
+  {
     const double ax = abs1(x);
     double err = 1.0;
 #pragma unroll
     for (int i = 4; i >= 0; --i) err = fma(err, ax, abs1(c[i]));
     if (abs1(p) <= 2.0 * kEps * err) return true;   // at the rounding floor
   }
-  const double dn = norm2(d);
-  const bool slope = dn > 0.0;               // p' = 0 (or NaN): no step, not converged -- as selects, not as a branch
-  const double inv = slope ? rcp1(dn) : 0.0;
-  const cd dx = mk(fma(p.x, d.x, p.y * d.y) * inv, fma(p.y, d.x, -(p.x * d.y)) * inv);
-  x = x - dx;
-  // stop rule: |dx|^3 <= 1e-13 |x| |dx_prev|^2, on magnitude keys (prev = key of the previous step, 0 before the first)
-  const int ks = mag_key(dx);
-  bool conv = false;
-  if (check) conv = slope && (3 * ks + kKeyMargin <= kKeyStop + mag_key(x) + 2 * prev);
+  const int ks = newton_move(p, d, x);
+  const bool conv = newton_converged(ks, prev, x);
   prev = ks;
   return conv;
 }
@@ -403,13 +411,21 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
   // sweeps 0 and 1: every root needs them (the stop rule wants two steps), so all five chains run unconditionally
   // and interleave (instruction-level parallelism); a step on an already converged root is harmless
   // (a rolled loop of two sweeps: one copy of the five interleaved chains keeps the hot loop inside the instruction cache)
+  int kfirst[4];   // key of the first step of each chain
+#pragma unroll
+  for (int k = 0; k < 4; ++k) kfirst[k] = 0;
 #pragma unroll 1
   for (int it = 0; it < 2; ++it) {
-    unsigned dn = 0;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) dn |= newton_step<false>(c, r[k], prev[k], it != 0) ? (1u << k) : 0u;
-    done |= dn;
+    for (int k = 0; k < 4; ++k) {
+      cd p, d;
+      horner_pd(c, r[k], p, d);
+      kfirst[k] = prev[k];
+      prev[k] = newton_move(p, d, r[k]);
+    }
   }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) done |= newton_converged(prev[k], kfirst[k], r[k]) ? (1u << k) : 0u;
   // The FIFTH root is not iterated: it follows from Vieta's sum, r4 = -c4 - (r0 + r1 + r2 + r3).  centre_seeds() puts the
   // root of largest modulus last, so the rounding of the sum (a few ulp of the LARGEST root) is a relative error of
   // a few ulp of r4 itself; the product of the five roots then verifies the solve.  v5 = that short cut is still on
@@ -471,7 +487,7 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
 #pragma unroll
       for (int j = 1; j < 5; ++j)
         if (j == k) { x = r[j]; pv = prev[j]; }
-      const bool cv = newton_step<true>(c, x, pv);
+      const bool cv = newton_step_floor(c, x, pv);
 #pragma unroll
       for (int j = 0; j < 5; ++j)
         if (j == k) { r[j] = x; prev[j] = pv; }
