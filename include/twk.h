@@ -61,7 +61,11 @@ typedef struct {
   int64_t handoff_slots; /* slots of the hand-over arena through which the first iteration (64 records, interval     */
                         /* pieces, seeds; 14,720 B per slot) of an unfinished source passes to the refinement stage  */
                         /* instead of being recomputed there.  -1 = default min(max_sources, 524288); 0 = none.      */
-                        /* Sources beyond the slots are still refined (their first iteration is recomputed).        */
+                        /* Sources beyond the slots are still refined (their first iteration is recomputed).  A context */
+                        /* with slots also gets 1024 carry-over slots (120 KB each) through which a source that fills */
+                        /* the 512-sample refinement stage takes its whole state to the 4096-sample stage; with 0     */
+                        /* (or beyond 1024 such sources per call) that stage recomputes the source from its first     */
+                        /* sample.                                                                                    */
   double slope_gate;    /* slope detector: at a change of the image count between adjacent samples the    */
                         /* new real pair must be perpendicular (within 45 deg) to the neighbouring ghost pair, else    */
                         /* it is re-judged as ghosts.  Applied only when both pairs are closer than slope_gate         */

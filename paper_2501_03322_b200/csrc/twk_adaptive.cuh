@@ -15,6 +15,33 @@ TWK_NOINLINE Piece eval_interval_cold(RecRef A, RecRef B, double dth, double slo
   return eval_interval(A, B, dth, slope_gate2, slope_cos2);
 }
 
+// Stage 2 -> stage 3 carry-over of a source that filled stage 2's capacity (rare: out of line).  Slot layout: carry_doubles().
+// Records of id < 64 of a handed-over source are still in its hand-over slot ([26][64]), the others in the CTA's arena.
+TWK_NOINLINE void carry_out(double* cs, int C, int n, const double* theta, const double* dA, const double* er,
+                            const uint16_t* ids, const double* arena, const double* hand, int status_bits) {
+  const int t = threadIdx.x;
+  for (int id = t; id < n; id += blockDim.x) {
+    const RecRef r = (hand && id < 64) ? RecRef{const_cast<double*>(hand) + id, 64}
+                                       : RecRef{const_cast<double*>(arena) + (size_t)id * kRecDoubles, 1};
+    double* d = cs + (size_t)id * kRecDoubles;
+#pragma unroll 2
+    for (int e = 0; e < kRecDoubles; ++e) d[e] = r.at(e);
+  }
+  double* cth = cs + (size_t)C * kRecDoubles;
+  uint16_t* cid = reinterpret_cast<uint16_t*>(cth + 3 * (size_t)C);
+  for (int i = t; i < n; i += blockDim.x) {
+    cth[i] = theta[i];
+    cth[C + i] = dA[i];
+    cth[2 * C + i] = er[i];
+    cid[i] = ids[i];
+  }
+  if (t == 0) {
+    double* hd = cs + (size_t)C * (kRecDoubles + 3) + C / 4;
+    hd[0] = code_as_double(n);
+    hd[1] = code_as_double(status_bits);
+  }
+}
+
 struct AdaptArgs {
   Batch b;
   double tol;
@@ -33,17 +60,25 @@ struct AdaptArgs {
   const double* seeds;   // [kSeedDoubles][n_sources] seed blocks written by stage 0
   const double* handoff; // stage 2: hand-over arena written by stage 1 (null: recompute the first iteration)
   long long handoff_slots;   // worklist entries < handoff_slots have a hand-over slot
+  // carry-over arena between the refinement stages: a source that fills stage 2's capacity takes its whole state along
+  // (records, sorted angles, interval pieces) instead of being recomputed from its first sample by stage 3
+  double* carry;         // [carry_slots][carry_doubles(carry_cap)] or null
+  long long carry_slots; // entries of the next stage's worklist < carry_slots have a slot
+  int carry_cap;         // sample capacity of a slot (= stage 2's cap)
+  int carry_role;        // 0 none, 1 this stage writes slots (stage 2), 2 this stage reads them (stage 3)
   double* out_mu;
   double* out_err;       // may be null
   int32_t* out_nsamples; // may be null
   uint32_t* out_status;  // may be null
 };
 
+// carry-over slot, in doubles: records [C][26] | theta [C] | dA [C] | err [C] | ids [C] u16 | header [8]: n, status bits
+__host__ __device__ inline size_t carry_doubles(int C) { return (size_t)C * (kRecDoubles + 3) + (size_t)C / 4 + 8; }
 constexpr int kScrDoubles = 20;   // per-thread scratch of point_solve_cs<true> (roots and residuals of the five roots)
 __host__ __device__ inline size_t adaptive_smem_bytes(int cap, bool scr, bool tile) {
   // (with a tile the scratch of the point solves is the tile column the record goes to)
   size_t doubles = 3 * (size_t)cap + 2 * kThreads + 8 + 32 + (scr && !tile ? kScrDoubles * kThreads : 0) + (tile ? kRecDoubles * kThreads : 0);
-  size_t ints = 2 * kThreads + 4;
+  size_t ints = 2 * kThreads + 8;
   return doubles * 8 + ints * 4 + (size_t)cap * 2;
 }
 
@@ -70,19 +105,22 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   double* tile = scrbuf + (kScr && !kTile ? kScrDoubles * kThreads : 0);   // [26][64] (kTile) records of this iteration's new samples
   int* newint = reinterpret_cast<int*>(tile + (kTile ? kRecDoubles * kThreads : 0));   // [64] interval of quantile k
   int* cint = newint + kThreads;    // [64] compacted
-  int* iscr = cint + kThreads;      // [4]
-  uint16_t* ids = reinterpret_cast<uint16_t*>(iscr + 4);   // [cap] arena id of the sample at each sorted position
+  int* iscr = cint + kThreads;      // [8]: current entry, two warp counts, slope count, -, carry-over slot
+  uint16_t* ids = reinterpret_cast<uint16_t*>(iscr + 8);   // [cap] arena id of the sample at each sorted position
 
   const int t = threadIdx.x;
   const int lane = t & 31, warp = t >> 5;
   double* arena = p.arena + (size_t)blockIdx.x * (size_t)cap * kRecDoubles;
   // record of sample id: ids 0..63 of a handed-over source live in its hand-over slot ([26][64]), the rest in the arena
   const double* hand = nullptr;
+  const double* carried = nullptr;   // stage 3: records 0 .. n_carried - 1 of a carried-over source live in its slot
+  int n_carried = 0;
   int tile_base = 1 << 30;   // ids >= tile_base are in the tile (the current iteration's new samples)
   auto recref = [&](int id) -> RecRef {
     TWK_CHECK(id >= 0 && id < cap, 0);
     if (kTile && id >= tile_base) return RecRef{tile + (id - tile_base), kThreads};
     if (hand && id < kThreads) return RecRef{const_cast<double*>(hand) + id, kThreads};
+    if (id < n_carried) return RecRef{const_cast<double*>(carried) + (size_t)id * kRecDoubles, 1};
     return RecRef{arena + (size_t)id * kRecDoubles, 1};
   };
   // L-4 guard term of interval (i, i + 1) in a sorted list of nn samples (neighbours i - 1 and i + 2, cyclic)
@@ -158,6 +196,27 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
       if (t < kSeedDoubles) seeds[t] = p.seeds[(size_t)t * (size_t)p.b.n_sources + (size_t)src];
     }
     uint32_t status = S.status;
+    carried = nullptr;
+    n_carried = 0;
+    // (compile-time roles: the stage-2 instance of the kernel is the one with the tile and only writes slots, the
+    //  stage-3 instance only reads them; neither carries the other's code)
+    if (!kTile && p.carry_role == 2 && cur < p.carry_slots) {   // carried over from stage 2: continue where it stopped
+      const int C = p.carry_cap;
+      const double* cs = p.carry + (size_t)cur * carry_doubles(C);
+      const double* hd = cs + (size_t)C * (kRecDoubles + 3) + C / 4;
+      n = code_of(hd[0]);
+      status |= (uint32_t)code_of(hd[1]);
+      carried = cs;
+      n_carried = n;
+      const double* cth_ = cs + (size_t)C * kRecDoubles;
+      const uint16_t* cid = reinterpret_cast<const uint16_t*>(cth_ + 3 * (size_t)C);
+      for (int i = t; i < n; i += kThreads) {
+        theta[i] = cth_[i];
+        dA[i] = cth_[C + i];
+        er[i] = cth_[2 * C + i];
+        ids[i] = cid[i];
+      }
+    }
     bool exhausted = false, slope_seen = false;
     double A = 0.0, E = 0.0;
     for (;;) {
@@ -423,6 +482,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         const int slot = atomicAdd(p.next_count, 1);
         TWK_CHECK(slot >= 0 && slot < p.b.n_sources, 4);
         p.next_list[slot] = (int32_t)src;
+        if (kTile) iscr[5] = slot;
       } else {
         if (exhausted) status |= 2u;
         if (rep) status |= 4u;
@@ -433,6 +493,13 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         if (p.out_nsamples) p.out_nsamples[src] = n;
         if (p.out_status) p.out_status[src] = status;
       }
+    }
+    if (kTile && exhausted && !p.final_stage && p.carry_role == 1) {   // (uniform) the state goes along to the next stage
+      __syncthreads();
+      const long long slot = iscr[5];
+      if (slot < p.carry_slots && n <= p.carry_cap)
+        carry_out(p.carry + (size_t)slot * carry_doubles(p.carry_cap), p.carry_cap, n, theta, dA, er, ids, arena, hand,
+                  (int)((status & ~S.status) | (rep ? 4u : 0u) | (nonf ? 16u : 0u) | ((slope_seen || slp) ? 32u : 0u)));
     }
   }
 }

@@ -19,6 +19,7 @@ constexpr int kStage2Cap = 512;         // sample capacity of refinement stage 2
 constexpr int kStage2CtasPerSM = 6;
 constexpr int kStage3CtasPerSM = 2;
 constexpr int kFixedTile = 128;
+constexpr size_t kCarrySlots = 1024;    // stage 2 -> stage 3 carry-over slots (120 KB each); beyond them stage 3 recomputes
 constexpr size_t kDefaultHandoffSlots = size_t(1) << 19;   // 524,288 slots x 14,592 B = 7.6 GB
 
 thread_local char g_cuda_msg[256] = "";
@@ -50,8 +51,8 @@ size_t handoff_slots(const twk_options& o, size_t max_sources) {
 }
 
 struct Layout {
-  size_t counters, list1, list2, seeds, handoff, arena, total;
-  size_t slots;
+  size_t counters, list1, list2, seeds, handoff, carry, arena, total;
+  size_t slots, carry_slots;
 };
 Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
   const Plan P = make_plan(o, sms);
@@ -63,6 +64,9 @@ Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
   L.list2 = off;    off += align256(max_sources * 4);
   L.seeds = off;    off += align256(max_sources * twk::kSeedDoubles * 8);
   L.handoff = off;  off += align256(L.slots * twk::kHandDoubles * 8);
+  // (a context without hand-over slots is the lean one: no carry-over either)
+  L.carry_slots = (P.cap2 && P.cap3 && L.slots) ? (kCarrySlots < max_sources ? kCarrySlots : max_sources) : 0;
+  L.carry = off;    off += align256(L.carry_slots * twk::carry_doubles(P.cap2 ? P.cap2 : 1) * 8);
   L.arena = off;    off += align256(P.arena_doubles * 8);
   L.total = off;
   return L;
@@ -340,6 +344,10 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a2.next_count = counters + 3;
     a2.handoff = handoff;
     a2.handoff_slots = (long long)ctx->lay.slots;
+    a2.carry = reinterpret_cast<double*>(ctx->ws + ctx->lay.carry);
+    a2.carry_slots = (long long)ctx->lay.carry_slots;
+    a2.carry_cap = P.cap2;
+    a2.carry_role = (P.cap3 && ctx->lay.carry_slots) ? 1 : 0;
     constexpr bool kScr2 = kStage2Scr, kTile2 = kStage2Tile;
     const size_t smem2 = twk::adaptive_smem_bytes(P.cap2, kScr2, kTile2);
     if (a2.guard) twk::adaptive_kernel<true, kScr2, kTile2><<<P.grid2, twk::kThreads, smem2, stream>>>(a2);
@@ -354,6 +362,10 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a3.list = list2;
     a3.count = counters + 3;
     a3.cursor = counters + 4;
+    a3.carry = reinterpret_cast<double*>(ctx->ws + ctx->lay.carry);
+    a3.carry_slots = (long long)ctx->lay.carry_slots;
+    a3.carry_cap = P.cap2;
+    a3.carry_role = (P.cap2 && ctx->lay.carry_slots) ? 2 : 0;
     const size_t smem3 = twk::adaptive_smem_bytes(P.cap3, false, false);
     if (a3.guard) twk::adaptive_kernel<true, false, false><<<P.grid3, twk::kThreads, smem3, stream>>>(a3);
     else twk::adaptive_kernel<false, false, false><<<P.grid3, twk::kThreads, smem3, stream>>>(a3);

@@ -95,13 +95,22 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   const cd zeta = mk(fma(rho, cs, zc.x), fma(rho, sn, zc.y));
   const cd dzeta = mk(-rho * sn, rho * cs);                     // zeta' = i rho e^{i theta}
   cd y = mk(zeta.x - L.z2, zeta.y);
-  // next to a lens (closer than 1e-8 s) one root runs off towards infinity and one onto the pole: such a sample is left
-  // to the cold solver; ON the lens it is moved off it first (B-1)
-  const bool near_lens = fmin(norm2(y), norm2(mk(y.x + L.s, y.y))) < 1e-16 * L.s * L.s;
-  bool guarded = false;
-  if (near_lens) guarded = lens_guard(y, L.s);
   cd c[6], eta[5];
   coeffs_eq6(y, L.s, L.m2, c);
+  // next to a lens (closer than ~1e-8 s) one root runs off towards infinity and one onto the pole: such a sample is left
+  // to the cold solver; ON the lens it is moved off it first (B-1).  |c5| = |y| |y + s| measures the distance to the
+  // nearer lens (the other factor is within [s/2, ...]): |c5| < 1e-8 s^2 <=> closer than (1..2) 1e-8 s
+  const double n5 = norm2(c[5]), s2 = L.s * L.s;
+  const bool near_lens = !(n5 >= 1e-16 * (s2 * s2));
+  bool guarded = false;
+  if (near_lens) {
+    guarded = lens_guard(y, L.s);
+    if (guarded) {
+      const Coef6 C = coeffs_eq6_cold(y, L.s, L.m2);
+#pragma unroll
+      for (int i = 0; i < 6; ++i) c[i] = C.c[i];
+    }
+  }
   int solved = 0;
   if (seeds && !near_lens) {
     const double dx = rho * cs, dy = rho * sn;                  // delta
@@ -114,7 +123,8 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
       eta[k] = mk(fma(pxx, dx, fma(pxy, dy, ex)), fma(pyx, dx, fma(pyy, dy, ey)));
     }
     {   // the seeded solve works on the monic quintic; the cold solver below gets the same coefficients with c5 = 1
-      const cd i5 = crecip(c[5]);
+      const double r5 = rcp(n5);
+      const cd i5 = mk(c[5].x * r5, -c[5].y * r5);
 #pragma unroll
       for (int i = 0; i < 5; ++i) c[i] = c[i] * i5;
       c[5] = mk(1.0, 0.0);
@@ -231,13 +241,16 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     flags |= kPointRepaired;
   }
   // record: positives to slots 0.., negatives to slots 2..: the slot of a root is the number of same-parity roots before it
+  int sp = 0, sm = 2;
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
     const cd z = mk(eta[k].x + L.z2, eta[k].y);
     const bool isp = posm >> k & 1u, isn = negm >> k & 1u;
     if (out_z) { out_z[2 * k] = z.x; out_z[2 * k + 1] = z.y; }
     if (out_kind) out_kind[k] = (int8_t)(isp ? 1 : (isn ? -1 : 0));
-    const int slot = isp ? __popc(posm & ((1u << k) - 1u)) : 2 + __popc(negm & ((1u << k) - 1u));
+    const int slot = isp ? sp : sm;   // = the number of same-parity roots before this one (+ 2 for the negatives)
+    sp += isp ? 1 : 0;
+    sm += isn ? 1 : 0;
     // (slots stay inside the record whatever the kinds are: with non-finite J every root counts as negative)
     if ((isp || isn) && slot < (isp ? 2 : 5)) {
       const double invJ = rcp1(J[k]);   // (40 bits: z' and z'^z'' only enter the parabolic corrections and the estimates)
@@ -535,11 +548,12 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, const LinkConst& K,
   P.slope = 0;
   const bool a5 = A.nreal() == 5, b5 = B.nreal() == 5;
   int leftApos = -1, leftAneg = -1, leftBpos = -1, leftBneg = -1;
-  // links are collected first (slot of A | slot of B << 4, one byte each) and evaluated in ONE loop below
-  unsigned long long links = 0;
+  // links are collected first (slot of A | slot of B << 3, six bits each: five links fit one 32-bit word) and evaluated
+  // in ONE loop below
+  unsigned links = 0;
   int nl = 0;
   auto add_link = [&](int ka, int kb) {
-    links |= (unsigned long long)(ka | (kb << 4)) << (8 * nl);
+    links |= (unsigned)(ka | (kb << 3)) << (6 * nl);
     ++nl;
   };
   // ---- positive parity: slots 0,(1) --------------------------------------------------------------------
@@ -608,8 +622,8 @@ TWK_HD Piece eval_interval(const RecRef& A, const RecRef& B, const LinkConst& K,
   // ---- a7: area and error of every link (one copy of the code; 3 or 4 or 5 trips) ----------------------------
 #pragma unroll 1
   for (int l = 0; l < nl; ++l) {
-    const int ka = (int)(links & 15u), kb = (int)((links >> 4) & 15u);
-    links >>= 8;
+    const int ka = (int)(links & 7u), kb = (int)((links >> 3) & 7u);
+    links >>= 6;
     link_terms(A, B, ka, kb, ka < 2 ? 1.0 : -1.0, K, P.dA, P.err);
   }
   // ---- caustic crossing: the extra (+,-) pair on the 5-image side connects to itself -------------

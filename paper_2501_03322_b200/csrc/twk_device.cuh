@@ -264,6 +264,11 @@ TWK_HD void quintic_roots(const cd (&c)[6], cd (&r)[5]) {
 // that must not sit in the middle of the hot loop's instruction stream.
 struct Coef6 { cd c[6]; };
 struct Roots5 { cd r[5]; };
+TWK_NOINLINE Coef6 coeffs_eq6_cold(cd y, double s, double m2) {   // (rebuilt after the B-1 guard moved y: rare)
+  Coef6 C;
+  coeffs_eq6(y, s, m2, C.c);
+  return C;
+}
 TWK_NOINLINE Roots5 quintic_roots_cold(Coef6 C) {
   Roots5 R;
   quintic_roots(C.c, R.r);
@@ -350,7 +355,7 @@ TWK_NOINLINE SeededState seeded_recover(cd c0, cd c5, cd tot, SeededState S) {
 // spending FP64 multiplications on it.  NaN gives the largest key (never "converged"), zero gives 0.
 TWK_HD int mag_key(cd v) {
 #ifdef __CUDA_ARCH__
-  return (__double2hiint(abs1(v)) & 0x7fffffff) >> 4;
+  return (int)((unsigned)__double2hiint(abs1(v)) >> 4);   // (unsigned: a NaN of either sign is the largest key)
 #else
   return 0;
 #endif

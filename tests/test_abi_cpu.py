@@ -29,9 +29,11 @@ def test_workspace_bytes_is_host_arithmetic():
     a = P.twk_workspace_bytes(1000)
     b = P.twk_workspace_bytes(4096000)
     assert 0 < a < b < 1 << 34
-    # the hand-over arena (14,720 B per slot, default min(max_sources, 2^19) slots) is the bulk of a large context
+    # the hand-over arena (14,720 B per slot, default min(max_sources, 2^19) slots) is the bulk of a large context; with it
+    # come the 1024 carry-over slots between the refinement stages (512 samples x (26 + 3) doubles + ids + header)
     lean = P.twk_workspace_bytes(4096000, handoff_slots=0)
-    assert lean < 1 << 31 and b - lean == (1 << 19) * 14720
+    carry_slot = (512 * 29 + 512 // 4 + 8) * 8
+    assert lean < 1 << 31 and b - lean == (1 << 19) * 14720 + 1024 * carry_slot
     assert P.twk_workspace_bytes(1000, handoff_slots=-2) == 0        # invalid
     assert P.twk_workspace_bytes(1000, max_samples=512) < a          # no stage-3 arena
     assert P.twk_workspace_bytes(1000, max_samples=5000) == 0        # invalid options

@@ -441,6 +441,37 @@ def test_lightcurve_orbital_motion(ctx):
     assert neg.any() and np.all(np.isnan(mub[neg])) and np.all(stb[neg] & 8) and np.all(np.isfinite(mub[mid != 0]))
 
 
+def test_stage3_carry_over_matches_recompute():
+    """A source that fills stage 2's 512 samples takes its state along to stage 3 (carry-over slots); a lean context
+    (handoff_slots = 0: no slots at all) recomputes such a source from its first sample instead.  Same method, same
+    answers: statuses equal, magnifications equal to rounding-level ties of the sampler, and like-for-like with the oracle."""
+    import paper_2501_03322_b200 as P
+    wl = W.config2().subset(np.arange(4940, 5070))          # the central-caustic crossing of config 2
+    tol = 1e-7
+    a = P.Context(4096)
+    ga = a.magnify_workload(wl, tol)
+    sa = a.twk_last_stats()
+    a.close()
+    b = P.Context(4096, handoff_slots=0)
+    gb = b.magnify_workload(wl, tol)
+    sb = b.twk_last_stats()
+    b.close()
+    assert sa["n_stage3"] >= 10 and sa["n_stage3"] == sb["n_stage3"]
+    assert np.array_equal(ga["status"], gb["status"])
+    d = np.abs(ga["mu"] / gb["mu"] - 1)
+    # (the lean context also recomputes the FIRST iteration, with interval widths theta_{i+1} - theta_i instead of the
+    #  constant 2 pi / 64: last-bit differences that move quantile ties, far below the tolerance)
+    assert np.median(d) < 1e-10 and d.max() < 10 * tol
+    # (at ~2000 samples per source the two runs stop within an iteration or two of each other)
+    assert np.all(np.abs(ga["nsamples"] - gb["nsamples"]) <= 128)
+    o = api.magnify(wl, tol, mode=0)
+    do = np.abs(ga["mu"] / o["mu"] - 1)
+    assert np.array_equal(ga["status"].astype(np.uint32) & 3, o["status"] & 3)
+    assert np.quantile(do, 0.9) < 1e-9 and do.max() < 10 * tol
+    ref = api.magnify(wl, 1e-8, mode=1)
+    assert np.abs(ga["mu"] / ref["mu"] - 1).max() <= 2 * tol
+
+
 def test_frame_option(ctx):
     """frame = 1: the caller's zeta has the primary at the origin (BASELINE configs 1, 2); the library adds z1."""
     import paper_2501_03322_b200 as P
