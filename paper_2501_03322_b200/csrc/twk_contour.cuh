@@ -156,12 +156,12 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     const double ia_ = rab * nb, ib_ = rab * na;
     const cd a = mk(za.x * ia_, -za.y * ia_), b = mk(zb.x * ib_, -zb.y * ib_);
     const cd a2 = a * a, b2 = b * b;
-    const cd f = L.m1 * a + L.m2 * b;                    // Eq.(7)
-    fp[k] = L.m1 * a2 + L.m2 * b2;
+    fp[k] = L.m1 * a2 + L.m2 * b2;                       // Eq.(7)
     a3[k] = a2 * a;                                      // f'' is finished below, for the real images only
     b3[k] = b2 * b;
-    Res[k] = mk(y.x - eta[k].x - f.x, y.y - eta[k].y + f.y);   // Eq.(12): y - eta - conj(f)
-    J[k] = 1.0 - norm2(fp[k]);                           // Eq.(7)
+    // Eq.(12): R = y - eta - conj(f), f = m1 a + m2 b folded into the subtraction
+    Res[k] = mk(fma(-L.m1, a.x, fma(-L.m2, b.x, y.x - eta[k].x)), fma(L.m1, a.y, fma(L.m2, b.y, y.y - eta[k].y)));
+    J[k] = fma(-fp[k].x, fp[k].x, fma(-fp[k].y, fp[k].y, 1.0));   // Eq.(7): 1 - |f'|^2
     R2[k] = norm2(Res[k]);
   }
   {   // all ten finite?  |R|^2 >= 0 and J <= 1: their sums cannot cancel an infinity and NaN propagates
@@ -242,6 +242,7 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
   }
   // record: positives to slots 0.., negatives to slots 2..: the slot of a root is the number of same-parity roots before it
   int sp = 0, sm = 2;
+  const double m1x2 = L.m1 + L.m1, m2x2 = L.m2 + L.m2, rho2 = rho * rho;
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
     const cd z = mk(eta[k].x + L.z2, eta[k].y);
@@ -255,12 +256,13 @@ TWK_HD int point_solve_cs(const Lens& L, cd zc, double rho, double cs, double sn
     if ((isp || isn) && slot < (isp ? 2 : 5)) {
       const double invJ = rcp1(J[k]);   // (40 bits: z' and z'^z'' only enter the parabolic corrections and the estimates)
       // z' = (zeta' - conj(f') conj(zeta')) / J                       Eq.(10), repaired (E-2)
-      const cd t = conj(fp[k]) * conj(dzeta);
-      const cd zp = mk((dzeta.x - t.x) * invJ, (dzeta.y - t.y) * invJ);
-      // z'^z'' = (rho^2 + Im[z'^2 zeta' f'']) / J                     Eq.(10), repaired (E-3)
-      const cd fpp = 2.0 * (L.m1 * a3[k] + L.m2 * b3[k]);
-      const cd u = (zp * zp) * (dzeta * fpp);
-      const double w = fma(rho, rho, u.y) * invJ;
+      // (conj(f') conj(zeta') = conj(f' zeta'), folded into the subtraction)
+      const cd zp = mk(fma(fp[k].y, dzeta.y, fma(-fp[k].x, dzeta.x, dzeta.x)) * invJ,
+                       fma(fp[k].x, dzeta.y, fma(fp[k].y, dzeta.x, dzeta.y)) * invJ);
+      // z'^z'' = (rho^2 + Im[z'^2 zeta' f'']) / J                     Eq.(10), repaired (E-3);  f'' = 2 (m1 a^3 + m2 b^3)
+      const cd fpp = mk(fma(m1x2, a3[k].x, m2x2 * b3[k].x), fma(m1x2, a3[k].y, m2x2 * b3[k].y));
+      const cd zp2 = zp * zp, zf = dzeta * fpp;
+      const double w = fma(zp2.x, zf.y, fma(zp2.y, zf.x, rho2)) * invJ;
       rec.at(kZX + slot) = z.x;
       rec.at(kZY + slot) = z.y;
       rec.at(kPX + slot) = zp.x;

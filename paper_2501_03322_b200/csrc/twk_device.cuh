@@ -126,18 +126,15 @@ TWK_HD void coeffs_eq6(cd y, double s, double m2, cd c[6]) {
   // c4 = (conj(y) y - 1 - 2 s conj(y)) v_c + m2 s
   {
     const cd t = mk(yy - 1.0 - 2.0 * s * yb.x, -2.0 * s * yb.y);
-    const cd u = t * vc;
-    c[4] = mk(u.x + m2s, u.y);
+    c[4] = cfma(t, vc, mk(m2s, 0.0));
   }
   // c3 = (2y - s) [v_p v_c + 2 i Im y - m2 s] + 4 i (m2 s - y) Im y
   {
     const cd a = mk(2.0 * y.x - s, 2.0 * y.y);
-    cd b = vp * vc;
-    b.x -= m2s;
-    b.y += 2.0 * Iy;
+    const cd b = cfma(vp, vc, mk(-m2s, 2.0 * Iy));
     const cd d = mk(m2s - y.x, -y.y);           // (m2 s - y)
     const cd e = mk(-4.0 * Iy * d.y, 4.0 * Iy * d.x);   // 4 i Im(y) (m2 s - y)
-    c[3] = a * b + e;
+    c[3] = cfma(a, b, e);
   }
   // c2 = Re(v_p)^2 Re(v_c) + i Im(y) Re(v_p) Re(1 - s y) + s Im(y)^2 (2 + s v_c) + m2 s [2 conj(y)(y - s) - (1 - s y)]
   {
@@ -151,9 +148,7 @@ TWK_HD void coeffs_eq6(cd y, double s, double m2, cd c[6]) {
   // c1 = m2 s [(s + 2y) v_p + s (2 i s Im y - m2)]
   {
     const cd a = mk(s + 2.0 * y.x, 2.0 * y.y);
-    cd t = a * vp;
-    t.x += -s * m2;
-    t.y += 2.0 * s * s * Iy;
+    const cd t = cfma(a, vp, mk(-s * m2, 2.0 * s * s * Iy));
     c[1] = m2s * t;
   }
   // c0 = s^2 m2^2 y
@@ -360,6 +355,13 @@ TWK_HD int mag_key(cd v) {
   return 0;
 #endif
 }
+TWK_HD int mag_key1(double v) {   // key of a non-negative (or NaN) real
+#ifdef __CUDA_ARCH__
+  return (int)((unsigned)__double2hiint(v) >> 4);
+#else
+  return 0;
+#endif
+}
 constexpr int kKeyOne = 1023 << 16;                  // key of 1.0
 constexpr int kKeyStop = (0x3d3c2000 >> 4) - kKeyOne;   // 2^16 log2(TWK_STOP_FACTOR * eps) = 2^16 log2(1e-13)
 constexpr int kKeyMargin = 1 << 16;                  // the piecewise-linear log2 (< 0.09 per key): a factor 2 on |dx|^3 covers it
@@ -380,9 +382,9 @@ TWK_HD void horner_pd(const cd (&c)[6], cd x, cd& p, cd& d) {
 // "converges" is what the Vieta recovery replaces.
 TWK_HD int newton_move(cd p, cd d, cd& x) {
   const double inv = rcp1(norm2(d));
-  const cd dx = mk(fma(p.x, d.x, p.y * d.y) * inv, fma(p.y, d.x, -(p.x * d.y)) * inv);
-  x = x - dx;
-  return mag_key(dx);
+  const cd num = mk(fma(p.x, d.x, p.y * d.y), fma(p.y, d.x, -(p.x * d.y)));   // p conj(p'):  dx = num / |p'|^2
+  x = mk(fma(-num.x, inv, x.x), fma(-num.y, inv, x.y));
+  return mag_key1(abs1(num) * inv);   // |dx|_1 = (|Re num| + |Im num|) / |p'|^2
 }
 // stop rule: |dx|^3 <= 1e-13 |x| |dx_prev|^2 on magnitude keys (kprev = 0: no previous step, only dx = 0 passes)
 TWK_HD bool newton_converged(int ks, int kprev, cd x) { return 3 * ks + kKeyMargin <= kKeyStop + mag_key(x) + 2 * kprev; }
