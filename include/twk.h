@@ -170,6 +170,12 @@ int twk_images_fixed_seeded(twk_ctx* ctx, size_t n_models, const double* s, cons
 int twk_stage1_records(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho, size_t n_sources,
                        const int32_t* model_id, const double* zeta, double* out_records, uint32_t* out_diag, void* stream);
 
+/* Diagnostics for the parity harness (SURVEY T-1): the Eq.(6) coefficients c0..c5 of the point source at zeta,
+ * exactly as the device builder of the kernels computes them (planet frame; before the monic normalisation).
+ *   out_c   DEVICE double[n_sources][6][2]  (re, im) of c0..c5.  Same batch arguments as twk_magnify (rho is not read). */
+int twk_coeffs_eq6(twk_ctx* ctx, size_t n_models, const double* s, const double* q, size_t n_sources, const int32_t* model_id,
+                   const double* zeta, double* out_c, void* stream);
+
 /* End-to-end convenience with HOST buffers (same meaning as twk_magnify): copies the inputs host->device into the
  * context's staging area, runs twk_magnify on `stream`, copies the outputs device->host and synchronises the
  * stream before returning.  Optional outputs may be NULL. */

@@ -19,7 +19,7 @@ TWK_ST_CONVERGED, TWK_ST_CAP, TWK_ST_REPAIRED, TWK_ST_DOMAIN, TWK_ST_NUMERIC, TW
 
 SYMBOLS = ["twk_default_options", "twk_create", "twk_destroy", "twk_workspace_bytes", "twk_magnify", "twk_magnify_lightcurve", "twk_magnify_lightcurve_orbital",
            "twk_images_fixed", "twk_images_fixed_seeded", "twk_stage1_records",
-           "twk_magnify_host", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_debug_counters", "twk_strerror", "twk_version"]
+           "twk_coeffs_eq6", "twk_magnify_host", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_debug_counters", "twk_strerror", "twk_version"]
 
 
 class TwkError(RuntimeError):
@@ -57,6 +57,7 @@ def lib():
         L.twk_images_fixed.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, vp]
         L.twk_images_fixed_seeded.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
         L.twk_stage1_records.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, vp, vp, vp]
+        L.twk_coeffs_eq6.argtypes = [vp, sz, vp, vp, sz, vp, vp, vp, vp]
         L.twk_last_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int), vp]
         L.twk_enable_stage_timing.argtypes = [vp, i32]
         L.twk_last_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
@@ -241,6 +242,16 @@ class Context:
         _check(lib().twk_stage1_records(self._h, int(s.shape[0]), _ptr(s), _ptr(q), _ptr(rho), n, _ptr(model_id), _ptr(zeta),
                                         _ptr(rec), _ptr(diag), _stream_ptr(stream)), "twk_stage1_records")
         return dict(records=rec, diag=diag)
+
+    def twk_coeffs_eq6(self, s, q, zeta, model_id=None, stream=None):
+        """Eq.(6) coefficients of the point source at every zeta as the device builder computes them: complex128[n, 6]."""
+        import torch
+        n = int(zeta.shape[0])
+        out = torch.zeros((n, 6, 2), dtype=torch.float64, device=zeta.device)
+        _check(lib().twk_coeffs_eq6(self._h, int(s.shape[0]), _ptr(s), _ptr(q), n, _ptr(model_id), _ptr(zeta), _ptr(out),
+                                    _stream_ptr(stream)), "twk_coeffs_eq6")
+        o = out.cpu().numpy()
+        return o[..., 0] + 1j * o[..., 1]
 
     # -- host-buffer call (end to end) -----------------------------------------------------------------------------
     def twk_magnify_host(self, s, q, rho, zeta, model_id=None, rel_tol=1e-4, out=None, stream=None):

@@ -455,6 +455,20 @@ int twk_stage1_records(twk_ctx* ctx, size_t n_models, const double* s, const dou
   return TWK_OK;
 }
 
+int twk_coeffs_eq6(twk_ctx* ctx, size_t n_models, const double* s, const double* q, size_t n_sources, const int32_t* model_id,
+                   const double* zeta, double* out_c, void* stream_) {
+  const int rc = check_batch(ctx, n_models, s, q, s /* rho is not read */, n_sources, model_id, zeta);
+  if (rc != TWK_OK) return rc;
+  if (n_sources == 0) return TWK_OK;
+  if (!out_c) return TWK_EINVAL;
+  const twk::Batch b{s, q, s, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame};
+  const long long want = ((long long)n_sources + 127) / 128;
+  const int grid = (int)(want < (long long)ctx->sms * 16 ? want : (long long)ctx->sms * 16);
+  twk::coeffs_kernel<<<grid, 128, 0, (cudaStream_t)stream_>>>(b, out_c);
+  TWK_CUDA(cudaGetLastError());
+  return TWK_OK;
+}
+
 int twk_magnify_host(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
                      size_t n_sources, const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu,
                      double* out_err, int32_t* out_nsamples, uint32_t* out_status, void* stream_) {

@@ -227,6 +227,23 @@ __global__ void __launch_bounds__(TILE) fixed_kernel(Batch b, int N, double* __r
 }
 
 // ------------------------------------------------------------------------------------------------------------
+// Parity harness: the Eq.(6) coefficients of the point source at zeta (twk_coeffs_eq6), one thread per source.
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) coeffs_kernel(Batch b, double* __restrict__ out_c) {
+  for (long long src = (long long)blockIdx.x * 128 + threadIdx.x; src < b.n_sources; src += (long long)gridDim.x * 128) {
+    const SourceParams S = load_source(b, src);
+    if (!S.valid) continue;
+    cd c[6];
+    coeffs_eq6(mk(S.zc.x - S.L.z2, S.zc.y), S.L.s, S.L.m2, c);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      out_c[src * 12 + 2 * i] = c[i].x;
+      out_c[src * 12 + 2 * i + 1] = c[i].y;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
 // FP64 FMA throughput probe: 8 independent DFMA chains per thread.
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) dfma_probe_kernel(int iters, double* __restrict__ out) {

@@ -476,6 +476,46 @@ def test_stage3_carry_over_matches_recompute():
     assert np.abs(ga["mu"] / ref["mu"] - 1).max() <= 2 * tol
 
 
+def test_device_coefficients_against_long_double(ctx):
+    """SURVEY T-1 on the device (a2): the Eq.(6) coefficients as the kernels build them (twk_coeffs_eq6) against
+    the oracle's long-double builder (itself pinned to the 60-digit elimination of Eq.(1)), coefficient by coefficient.
+    (i) The paper's regime: next to planetary caustics at q = 1e-7 .. 1e-4 the coefficients keep 12-14 digits in
+    FP64.  (ii) The whole validated domain of P:374 (0.1 <= s <= 10, q >= 1e-9): the small coefficients c1..c3
+    are differences of O(q s) terms there and no FP64 builder keeps more than ~eps / q of them; the device builder must be
+    as good as the oracle's own FP64 build of the same form."""
+    import torch
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to("cuda", torch.float64)
+
+    def errors(s, q, zc):
+        zeta = np.ascontiguousarray(np.stack([zc.real, zc.imag], 1))
+        g = ctx.twk_coeffs_eq6(f(s), f(q), f(zeta))
+        eg, eo = np.zeros((len(s), 6)), np.zeros((len(s), 6))
+        for i in range(len(s)):
+            ref = api.coeffs(float(s[i]), float(q[i]), complex(zc[i]), form=6, prec=1)
+            dbl = api.coeffs(float(s[i]), float(q[i]), complex(zc[i]), form=6, prec=0)
+            assert np.all(np.abs(ref) > 0)
+            eg[i] = np.abs(g[i] - ref) / np.abs(ref)
+            eo[i] = np.abs(dbl - ref) / np.abs(ref)
+        return eg, eo
+
+    rng = np.random.default_rng(61)
+    n = 2000
+    s = rng.uniform(0.4, 2.5, n)
+    q = 10.0 ** rng.uniform(-7, -4, n)
+    zc = (s - 1 / s) + np.sqrt(q) * (rng.uniform(-2, 2, n) + 1j * rng.uniform(-2, 2, n))
+    eg, eo = errors(s, q, zc)
+    # (2000 draws: the oracle's own FP64 build reaches 9e-12 in its worst case of this set, 1e-12 at the 99th percentile)
+    assert eg.max() < 2e-11 and eg.max() <= 4 * eo.max() and np.quantile(eg, 0.99) < 2e-12, (eg.max(), eo.max())
+    s = np.exp(rng.uniform(np.log(0.1), np.log(10.0), n))
+    q = 10.0 ** rng.uniform(-9, 0, n)
+    near = rng.random(n) < 0.7            # most of them on the planet's axis position s - 1/s, the rest anywhere
+    zc = np.where(near, (s - 1 / s) + np.sqrt(q) * (rng.uniform(-2, 2, n) + 1j * rng.uniform(-2, 2, n)),
+                  rng.uniform(-2, 2, n) + 1j * rng.uniform(-2, 2, n))
+    eg, eo = errors(s, q, zc)
+    assert eg.max() <= 4 * eo.max() and eg.max() < 1e-9, (eg.max(), eo.max())
+    assert np.all(np.median(eg, 0) <= 2 * np.median(eo, 0) + 1e-16), (np.median(eg, 0), np.median(eo, 0))
+    assert np.all(np.quantile(eg, 0.99, 0) <= 3 * np.quantile(eo, 0.99, 0) + 1e-15)
+
 def test_frame_option(ctx):
     """frame = 1: the caller's zeta has the primary at the origin (BASELINE configs 1, 2); the library adds z1."""
     import paper_2501_03322_b200 as P
