@@ -151,7 +151,8 @@ int twk_images_fixed(twk_ctx* ctx, size_t n_models, const double* s, const doubl
 /* Diagnostics for the parity harness: fixed sampling with the solver of the ADAPTIVE kernels.  As twk_images_fixed, but
  * every boundary sample is solved the way twk_magnify solves it: the point source at the
  * source centre is solved once, its five roots and their first-order response predict the roots of every boundary
- * sample, which are refined by Newton on the undeflated quintic, verified by Vieta's sums, recovered through Vieta's
+ * sample, which are refined by Newton on the undeflated (monic) quintic -- four chains, the fifth root from Vieta's sum --,
+ * verified by Vieta's product (and sum), recovered through Vieta's
  * formulas when two chains merge, with the cold Laguerre solver as last resort.
  *   out_diag   DEVICE uint32[4] or NULL: {point solves, Vieta recoveries, cold-solver fallbacks, lens-guard hits} */
 int twk_images_fixed_seeded(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,

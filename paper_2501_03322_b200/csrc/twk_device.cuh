@@ -415,9 +415,10 @@ TWK_HD int quintic_roots_seeded(const cd (&c)[6], cd (&r)[5], bool check_product
   for (int k = 0; k < 5; ++k) prev[k] = 0;
   const cd tot = -c[4];               // sum of the five roots (monic coefficients)
   unsigned done = 0;
-  // sweeps 0 and 1: every root needs them (the stop rule wants two steps), so all five chains run unconditionally
-  // and interleave (instruction-level parallelism); a step on an already converged root is harmless
-  // (a rolled loop of two sweeps: one copy of the five interleaved chains keeps the hot loop inside the instruction cache)
+  // sweeps 0 and 1: every root needs them (the stop rule wants two steps), so the four chains run unconditionally and
+  // interleave (instruction-level parallelism); a step on an already converged root is harmless.  A rolled loop of two
+  // sweeps (one copy of the four interleaved chains keeps the hot loop inside the instruction cache), no branch inside;
+  // the stop rule is evaluated once after it, from the keys of the two steps
   int kfirst[4];   // key of the first step of each chain
 #pragma unroll
   for (int k = 0; k < 4; ++k) kfirst[k] = 0;
