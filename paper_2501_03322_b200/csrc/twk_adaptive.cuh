@@ -75,9 +75,9 @@ struct AdaptArgs {
 // carry-over slot, in doubles: records [C][26] | theta [C] | dA [C] | err [C] | ids [C] u16 | header [8]: n, status bits
 __host__ __device__ inline size_t carry_doubles(int C) { return (size_t)C * (kRecDoubles + 3) + (size_t)C / 4 + 8; }
 constexpr int kScrDoubles = 20;   // per-thread scratch of point_solve_cs<true> (roots and residuals of the five roots)
-__host__ __device__ inline size_t adaptive_smem_bytes(int cap, bool scr, bool tile) {
+__host__ __device__ inline size_t adaptive_smem_bytes(int cap, bool scr, bool tile, int threads = kThreads) {
   // (with a tile the scratch of the point solves is the tile column the record goes to)
-  size_t doubles = 3 * (size_t)cap + 2 * kThreads + 8 + 32 + (scr && !tile ? kScrDoubles * kThreads : 0) + (tile ? kRecDoubles * kThreads : 0);
+  size_t doubles = 3 * (size_t)cap + 2 * kThreads + (threads > kThreads ? 16 : 8) + 32 + (scr && !tile ? kScrDoubles * kThreads : 0) + (tile ? kRecDoubles * kThreads : 0);
   size_t ints = 2 * kThreads + 8;
   return doubles * 8 + ints * 4 + (size_t)cap * 2;
 }
@@ -90,8 +90,16 @@ __host__ __device__ inline size_t adaptive_smem_bytes(int cap, bool scr, bool ti
 // kTile:  the records of the iteration's NEW samples are written twice, to the arena (where later iterations find them) and
 //         to a [26][64] shared-memory tile; the interval evaluations of the same iteration read every new record -- each
 //         thread's own, above all -- from the tile instead of waiting for the arena
-template <bool kGuard, bool kScr, bool kTile>
-__global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
+// TB:     threads per CTA.  64 = one thread per new sample (stage 2).  Stage 3 runs 128: the 64 new samples of an iteration
+//         are solved and their intervals evaluated by the first two warps as before, but the O(n) passes over the sorted
+//         state (sums, weight scan, shift) that dominate an iteration at thousands of samples are shared by four warps
+//         -- its 106 KB of shared memory allow two CTAs per SM whatever their width
+template <bool kGuard, bool kScr, bool kTile, int TB>
+__global__ void __launch_bounds__(TB, TB == kThreads ? 6 : 2) adaptive_kernel(AdaptArgs p) {
+  static_assert(TB % 32 == 0 && TB >= kThreads && TB <= 256, "TB");
+  constexpr int kWarps = TB / 32;
+  // "one of the 64 threads that own a new sample": always true at compile time when the CTA has no others
+#define TWK_FIRST64(tt) (TB == kThreads || (tt) < kThreads)
   extern __shared__ double sm[];
   const int cap = p.cap;
   double* theta = sm;            // [cap] sorted sample angles
@@ -99,8 +107,9 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
   double* er = dA + cap;         // [cap] error piece of interval (i, i+1)
   double* newth = er + cap;      // [64]  angle of quantile k
   double* cth = newth + kThreads;   // [64] compacted new angles
-  double* scratch = cth + kThreads; // [8]
-  double* seeds = scratch + 8;      // [30 (+2)] seed block of the source (twk_contour.cuh)
+  constexpr int kScanAt = (kWarps == 2) ? 4 : 8;   // scratch: block sums [0 .. 2 kWarps), warp totals of the scan behind them
+  double* scratch = cth + kThreads; // [8] (two warps) or [16]
+  double* seeds = scratch + 2 * kScanAt;   // [30 (+2)] seed block of the source (twk_contour.cuh)
   double* scrbuf = seeds + 32;      // [20][64] (kScr) scratch of the point solves
   double* tile = scrbuf + (kScr && !kTile ? kScrDoubles * kThreads : 0);   // [26][64] (kTile) records of this iteration's new samples
   int* newint = reinterpret_cast<int*>(tile + (kTile ? kRecDoubles * kThreads : 0));   // [64] interval of quantile k
@@ -183,14 +192,17 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
       {
         const char* hb = reinterpret_cast<const char*>(hand);
         asm volatile("prefetch.global.L2 [%0];" ::"l"(hb + t * 128));
-        if ((t + kThreads) * 128 < kHandDoubles * 8) asm volatile("prefetch.global.L2 [%0];" ::"l"(hb + (t + kThreads) * 128));
+        if (TB == kThreads && (t + kThreads) * 128 < kHandDoubles * 8)
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(hb + (t + kThreads) * 128));
       }
-      theta[t] = kTwoPi * double(t) / double(kThreads);
-      ids[t] = (uint16_t)t;
-      dA[t] = hand[kRecDoubles * kThreads + t];
-      er[t] = hand[(kRecDoubles + 1) * kThreads + t];
+      if (TWK_FIRST64(t)) {
+        theta[t] = kTwoPi * double(t) / double(kThreads);
+        ids[t] = (uint16_t)t;
+        dA[t] = hand[kRecDoubles * kThreads + t];
+        er[t] = hand[(kRecDoubles + 1) * kThreads + t];
+        flags |= recref(t).point_flags();
+      }
       if (t < kSeedDoubles) seeds[t] = hand[(kRecDoubles + 2) * kThreads + t];
-      flags |= recref(t).point_flags();
       n = kThreads;
     } else {      // not handed over: the loop below starts by inserting the 64 uniform samples into the empty list
       if (t < kSeedDoubles) seeds[t] = p.seeds[(size_t)t * (size_t)p.b.n_sources + (size_t)src];
@@ -210,7 +222,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
       n_carried = n;
       const double* cth_ = cs + (size_t)C * kRecDoubles;
       const uint16_t* cid = reinterpret_cast<const uint16_t*>(cth_ + 3 * (size_t)C);
-      for (int i = t; i < n; i += kThreads) {
+      for (int i = t; i < n; i += TB) {
         theta[i] = cth_[i];
         dA[i] = cth_[C + i];
         er[i] = cth_[2 * C + i];
@@ -223,17 +235,19 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
       __syncthreads();
       int m = kThreads;
       if (n == 0) {
-        cth[t] = kTwoPi * double(t) / double(kThreads);
-        cint[t] = -1;
+        if (TWK_FIRST64(t)) {
+          cth[t] = kTwoPi * double(t) / double(kThreads);
+          cint[t] = -1;
+        }
         __syncthreads();
       } else {
         // ---- area and error sums over all intervals (a7 reduction) ----------------------------------------------
         double a = 0.0, e = 0.0;
-        for (int i = t; i < n; i += kThreads) {
+        for (int i = t; i < n; i += TB) {
           a += dA[i];
           e += er[i];
         }
-        block_sum2(a, e, scratch);
+        block_sum2<kWarps>(a, e, scratch);
         A = a;
         E = e;
         const double tolA = p.tol * fabs(A);
@@ -243,18 +257,18 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         // ---- a8: error-weighted inverse-transform sampling, 64 quantiles ---------------------------
         const double avg = p.subtract_avg_tol ? tolA / double(n) : 0.0;   // "average tolerance", reading A-5
         double W = 0.0, unused = 0.0;
-        for (int i = t; i < n; i += kThreads) W += fmax(er[i] - avg, 0.0);
-        block_sum2(W, unused, scratch);
+        for (int i = t; i < n; i += TB) W += fmax(er[i] - avg, 0.0);
+        block_sum2<kWarps>(W, unused, scratch);
         const bool raw = !(W > 0.0);
         if (raw) W = E;
         const double scale = double(kThreads) / W;
         // Each interval marks the first quantile it owns (cint: interval | one-past-last quantile << 16, cth: its
         // exclusive cumulative weight); afterwards every quantile finds its owner by a max-scan over the marks and
         // computes its own angle: 64 angles in parallel even when one interval owns them all.
-        cint[t] = -1;
+        if (TWK_FIRST64(t)) cint[t] = -1;
         double carry = 0.0;
         __syncthreads();
-        for (int base = 0; base < n; base += kThreads) {
+        for (int base = 0; base < n; base += TB) {
           const int i = base + t;
           const double w = (i < n) ? (raw ? er[i] : fmax(er[i] - avg, 0.0)) : 0.0;
           double x = w;   // inclusive scan over the 64 threads
@@ -264,13 +278,26 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
             if (lane >= o) x += y;
           }
           __syncthreads();
-          if (lane == 31) scratch[4 + warp] = x;
+          if (lane == 31) scratch[kScanAt + warp] = x;
           __syncthreads();
-          const double w0 = scratch[4], w1 = scratch[5];
-          if (warp == 1) x += w0;
-          const double cum_incl = carry + x;
+          // prefix of the warps before this one, accumulated left to right: P_0 = 0, P_w = P_{w-1} + total_{w-1}
+          double before = 0.0, whole = 0.0;
+          if (kWarps == 2) {
+            const double w0 = scratch[kScanAt], w1 = scratch[kScanAt + 1];
+            if (warp == 1) before = w0;
+            whole = w0 + w1;
+          } else {
+#pragma unroll
+            for (int w2 = 0; w2 < kWarps; ++w2) {
+              if (w2 == warp) before = whole;
+              whole += scratch[kScanAt + w2];
+            }
+          }
+          const double cum_incl = carry + (x + before);
           double cum_excl = __shfl_up_sync(0xffffffffu, cum_incl, 1);
-          if (lane == 0) cum_excl = (warp == 0) ? carry : carry + w0;   // bitwise the left neighbour's cum_incl
+          // bitwise the left neighbour's cum_incl: the last lane of the warp before holds x = total_{w-1}, and
+          // total_{w-1} + P_{w-1} = P_w by construction (addition commutes exactly)
+          if (lane == 0) cum_excl = carry + before;
           if (w > 0.0) {
             // quantile k has target (k + 1/2)/64 * W (reading A-4); this interval owns those in [cum_excl, cum_incl)
             const int klo = min(kThreads, max(0, (int)ceil(cum_excl * scale - 0.5)));
@@ -280,20 +307,21 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
               cth[klo] = cum_excl;
             }
           }
-          carry += w0 + w1;
+          carry += whole;   // (= the last lane's x + before: the next tile's first cum_excl is this tile's last cum_incl)
         }
         __syncthreads();
         {
           // owner of quantile t: the last mark at a position <= t (inclusive max-scan over the 64 positions)
-          int pos = (cint[t] >= 0) ? t : -1;
+          int pos = (TWK_FIRST64(t) && cint[t] >= 0) ? t : -1;
   #pragma unroll
           for (int o = 1; o < 32; o <<= 1) {
             const int y = __shfl_up_sync(0xffffffffu, pos, o);
             if (lane >= o) pos = max(pos, y);
           }
-          if (lane == 31) iscr[1 + warp] = pos;
+          if (lane == 31 && TWK_FIRST64(t)) iscr[1 + warp] = pos;
           __syncthreads();
           if (warp == 1) pos = max(pos, iscr[1]);
+          if (!TWK_FIRST64(t)) pos = -1;
           int own = -1;
           double th = 0.0;
           if (pos >= 0) {
@@ -312,15 +340,17 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
             }
           }
           TWK_CHECK(own < 0 || th != th || (th > theta[own] && th < ((own + 1 < n) ? theta[own + 1] : kTwoPi)), 5);
-          newth[t] = th;
-          newint[t] = own;
+          if (TWK_FIRST64(t)) {
+            newth[t] = th;
+            newint[t] = own;
+          }
         }
         __syncthreads();
         // ---- drop invalid / duplicate angles, compact (ballot + prefix sum) --------------------------------------
-        bool v = (newint[t] >= 0) && (newth[t] == newth[t]);
+        bool v = TWK_FIRST64(t) && (newint[t] >= 0) && (newth[t] == newth[t]);
         if (v && t > 0 && newint[t - 1] == newint[t] && !(newth[t] > newth[t - 1])) v = false;
         const unsigned bal = __ballot_sync(0xffffffffu, v);
-        if (lane == 0) iscr[1 + warp] = __popc(bal);
+        if (lane == 0 && TWK_FIRST64(t)) iscr[1 + warp] = __popc(bal);
         __syncthreads();
         m = iscr[1] + iscr[2];
         const int rank = __popc(bal & ((1u << lane) - 1u)) + (warp ? iscr[1] : 0);
@@ -331,7 +361,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         __syncthreads();
         if (m == 0) { exhausted = true; break; }
         // ---- merge: old element j moves up by the number of new samples inserted before it ------------------------
-        for (int base = ((n - 1) / kThreads) * kThreads; base >= 0; base -= kThreads) {
+        for (int base = ((n - 1) / TB) * TB; base >= 0; base -= TB) {
           const int j = base + t;
           const bool have = j < n;
           double v0 = 0.0, v1 = 0.0, v2 = 0.0;
@@ -378,9 +408,9 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
 #ifdef TWK_DEBUG
       {   // the sorted list after the merge: angles strictly increasing, ids a permutation of 0 .. n_new - 1
         unsigned* bits = g_twk_stamp + (size_t)blockIdx.x * 128;
-        for (int i = t; i < 128; i += kThreads) bits[i] = 0u;
+        for (int i = t; i < 128; i += TB) bits[i] = 0u;
         __syncthreads();
-        for (int i = t; i < n_new; i += kThreads) {
+        for (int i = t; i < n_new; i += TB) {
           TWK_CHECK(i == 0 || theta[i] > theta[i - 1], 1);
           TWK_CHECK(theta[i] >= 0.0 && theta[i] < kTwoPi, 1);
           const unsigned id = ids[i];
@@ -424,7 +454,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
         for (int round = 0; round < 4096; ++round) {
           if (t == 0) iscr[3] = 0;
           __syncthreads();
-          for (int i = t; i < n; i += kThreads) {
+          for (int i = t; i < n; i += TB) {
             const int ib = (i + 1 < n) ? i + 1 : 0;
             const double dth = (i + 1 < n) ? theta[i + 1] - theta[i] : kTwoPi - theta[i];
             Piece P = eval_interval_cold(recref(ids[i]), recref(ids[ib]), dth, p.slope_gate2, p.slope_cos2);
@@ -444,7 +474,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
           if (nv == 0) break;
 #ifdef TWK_DEBUG
           unsigned* bits = g_twk_stamp + (size_t)blockIdx.x * 128;     // one writer per record per phase
-          for (int i = t; i < 128; i += kThreads) bits[i] = 0u;
+          for (int i = t; i < 128; i += TB) bits[i] = 0u;
           __syncthreads();
 #endif
           if (t < nv && (cint[t] & 256)) {
@@ -456,7 +486,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
           }
           __syncthreads();
 #ifdef TWK_DEBUG
-          for (int i = t; i < 128; i += kThreads) bits[i] = 0u;
+          for (int i = t; i < 128; i += TB) bits[i] = 0u;
           __syncthreads();
 #endif
           if (t < nv && !(cint[t] & 256)) {
@@ -503,5 +533,7 @@ __global__ void __launch_bounds__(kThreads, 6) adaptive_kernel(AdaptArgs p) {
     }
   }
 }
+
+#undef TWK_FIRST64
 
 }  // namespace twk

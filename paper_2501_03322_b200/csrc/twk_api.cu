@@ -18,6 +18,10 @@ constexpr bool kStage2Scr = true, kStage2Tile = true;
 constexpr int kStage2Cap = 512;         // sample capacity of refinement stage 2
 constexpr int kStage2CtasPerSM = 6;
 constexpr int kStage3CtasPerSM = 2;
+#ifndef TWK_S3_THREADS
+#define TWK_S3_THREADS 128
+#endif
+constexpr int kStage3Threads = TWK_S3_THREADS;   // four warps share the O(n) passes of a stage-3 iteration (twk_adaptive.cuh)
 constexpr int kFixedTile = 128;
 constexpr size_t kCarrySlots = 1024;    // stage 2 -> stage 3 carry-over slots (120 KB each); beyond them stage 3 recomputes
 constexpr size_t kDefaultHandoffSlots = size_t(1) << 19;   // 524,288 slots x 14,592 B = 7.6 GB
@@ -193,11 +197,11 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   }
   // opt in to the large dynamic shared memory of stage 3 (a per-function attribute shared by all contexts, so
   // always the maximum the build supports)
-  e = cudaFuncSetAttribute(twk::adaptive_kernel<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)twk::adaptive_smem_bytes(4096, false, false));
+  e = cudaFuncSetAttribute(twk::adaptive_kernel<false, false, false, kStage3Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)twk::adaptive_smem_bytes(4096, false, false, kStage3Threads));
   if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(twk::adaptive_kernel<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)twk::adaptive_smem_bytes(4096, false, false));
+    e = cudaFuncSetAttribute(twk::adaptive_kernel<true, false, false, kStage3Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)twk::adaptive_smem_bytes(4096, false, false, kStage3Threads));
   if (e != cudaSuccess) {
     cudaFree(c->ws);
     delete c;
@@ -350,8 +354,8 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a2.carry_role = (P.cap3 && ctx->lay.carry_slots) ? 1 : 0;
     constexpr bool kScr2 = kStage2Scr, kTile2 = kStage2Tile;
     const size_t smem2 = twk::adaptive_smem_bytes(P.cap2, kScr2, kTile2);
-    if (a2.guard) twk::adaptive_kernel<true, kScr2, kTile2><<<P.grid2, twk::kThreads, smem2, stream>>>(a2);
-    else twk::adaptive_kernel<false, kScr2, kTile2><<<P.grid2, twk::kThreads, smem2, stream>>>(a2);
+    if (a2.guard) twk::adaptive_kernel<true, kScr2, kTile2, twk::kThreads><<<P.grid2, twk::kThreads, smem2, stream>>>(a2);
+    else twk::adaptive_kernel<false, kScr2, kTile2, twk::kThreads><<<P.grid2, twk::kThreads, smem2, stream>>>(a2);
     ++launches;
     mark();
   }
@@ -366,9 +370,9 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     a3.carry_slots = (long long)ctx->lay.carry_slots;
     a3.carry_cap = P.cap2;
     a3.carry_role = (P.cap2 && ctx->lay.carry_slots) ? 2 : 0;
-    const size_t smem3 = twk::adaptive_smem_bytes(P.cap3, false, false);
-    if (a3.guard) twk::adaptive_kernel<true, false, false><<<P.grid3, twk::kThreads, smem3, stream>>>(a3);
-    else twk::adaptive_kernel<false, false, false><<<P.grid3, twk::kThreads, smem3, stream>>>(a3);
+    const size_t smem3 = twk::adaptive_smem_bytes(P.cap3, false, false, kStage3Threads);
+    if (a3.guard) twk::adaptive_kernel<true, false, false, kStage3Threads><<<P.grid3, kStage3Threads, smem3, stream>>>(a3);
+    else twk::adaptive_kernel<false, false, false, kStage3Threads><<<P.grid3, kStage3Threads, smem3, stream>>>(a3);
     ++launches;
     mark();
   }

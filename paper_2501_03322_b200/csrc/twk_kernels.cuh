@@ -113,8 +113,9 @@ __device__ __forceinline__ SourceParams load_source(const Batch& b, long long sr
   return P;
 }
 
-// block-wide sum of two doubles over kThreads (2 warps) -- result valid in every thread
-__device__ __forceinline__ void block_sum2(double& a, double& b, double* scratch /* >= 4 doubles */) {
+// block-wide sum of two doubles over kWarps warps -- result valid in every thread
+template <int kWarps = 2>
+__device__ __forceinline__ void block_sum2(double& a, double& b, double* scratch /* >= 2 kWarps doubles */) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     a += __shfl_xor_sync(0xffffffffu, a, o);
@@ -127,8 +128,13 @@ __device__ __forceinline__ void block_sum2(double& a, double& b, double* scratch
     scratch[2 * warp + 1] = b;
   }
   __syncthreads();
-  a = scratch[0] + scratch[2];
-  b = scratch[1] + scratch[3];
+  a = scratch[0];
+  b = scratch[1];
+#pragma unroll
+  for (int w = 1; w < kWarps; ++w) {
+    a += scratch[2 * w];
+    b += scratch[2 * w + 1];
+  }
 }
 
 // ------------------------------------------------------------------------------------------------------------
