@@ -26,7 +26,10 @@ namespace twk {
 // the stage-1 loop (which fills the 32 KB instruction cache by itself).
 // ------------------------------------------------------------------------------------------------------------
 constexpr int kS0Threads = 128;
-__global__ void __launch_bounds__(kS0Threads) seeds_kernel(Batch b, double* __restrict__ seeds) {
+// 6 blocks per SM at 80 registers (measured 2 / 3 / 4 / 5 / 6 / 8 blocks per SM at 195 / 168 / 128 / 96 / 80 / 64 registers:
+// 1.36 / 1.26 / 1.22 / 1.23 / 1.17 / 1.19 ms on config 3: the cold solver is one long dependent chain and wants warps more
+// than it minds a few spills)
+__global__ void __launch_bounds__(kS0Threads, 6) seeds_kernel(Batch b, double* __restrict__ seeds) {
   const long long n = b.n_sources;
   for (long long src = (long long)blockIdx.x * kS0Threads + threadIdx.x; src < n; src += (long long)gridDim.x * kS0Threads) {
     const SourceParams S = load_source(b, src);
