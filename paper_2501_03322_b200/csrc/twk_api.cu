@@ -113,7 +113,16 @@ void launch_stage1(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t
   long long group = (n_sources + resident - 1) / resident;
   group = group < 4 ? 4 : (group > twk::kS1Group ? twk::kS1Group : group);
   a.group = (int)group;
-  const long long groups = (n_sources + group - 1) / group;
+  long long groups = (n_sources + group - 1) / group;
+  // a large batch ends in small groups: its last two waves of 64-source groups go out as groups of 16, so that the
+  // resident CTAs finish within a quarter of a group's time of each other
+  a.n_big = groups;
+  a.tail_group = (int)group;
+  if (group == twk::kS1Group && groups > 8 * resident) {
+    a.n_big = groups - 2 * resident;
+    a.tail_group = 16;
+    groups = a.n_big + (n_sources - a.n_big * group + 15) / 16;
+  }
   const int grid = (int)(groups < resident ? groups : resident);
   if (a.guard) twk::stage1_kernel<true><<<grid, twk::kThreads, smem, stream>>>(a);
   else twk::stage1_kernel<false><<<grid, twk::kThreads, smem, stream>>>(a);

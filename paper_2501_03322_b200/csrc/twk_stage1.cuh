@@ -47,6 +47,8 @@ struct Stage1Args {
   int ps_test;           // N1: point-source adequacy tests in front of the contour path (twk_options.point_source_test)
   int guard;             // L-4 guard: hidden-crossing term in the interval estimates (twk_options.hidden_crossing_guard)
   int group;             // sources per group, 1..64 (smaller for small batches: more CTAs get work)
+  long long n_big;       // the first n_big groups have `group` sources, the rest of the batch goes out in groups of
+  int tail_group;        // `tail_group` sources: the last wave of a large batch ends together
   int final_stage;       // 1: there is no refinement stage (max_samples < 128): cap status instead of pending
   const double* seeds;   // [kSeedDoubles][n_sources] seed blocks written by stage 0
   int* cursor;           // group fetch counter (zeroed before launch)
@@ -95,8 +97,8 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
   const RecRef mine{recs + t, kThreads};
   const RecRef next{recs + ((t + 1) & (kThreads - 1)), kThreads};
   const long long n = p.b.n_sources;
-  const int G = p.group;
-  const long long n_groups = (n + G - 1) / G;
+  const long long n_big = p.n_big, n_in_big = n_big * p.group;
+  const long long n_groups = n_big + (n - n_in_big + p.tail_group - 1) / p.tail_group;
   int parity = 0;
 
   for (;;) {
@@ -105,7 +107,8 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
     __syncthreads();
     const long long g = iscr[0];
     if (g >= n_groups) break;
-    const long long base = g * G;   // first source of the group
+    const int G = (g < n_big) ? p.group : p.tail_group;
+    const long long base = (g < n_big) ? g * p.group : n_in_big + (g - n_big) * p.tail_group;   // first source of the group
     // ---- phase 1: parameters and centre roots of source base + t --------------------------------------------------
     {
       const long long src = base + t;
