@@ -1,8 +1,11 @@
-// twk_adaptive.cuh -- a8 + a9: the adaptive contour loop for one source per 64-thread CTA (refinement stages 2 and 3;
-// see twk_kernels.cuh).  A stage-2 source normally arrives with its first iteration done: stage 1 handed over its 64
-// records, 64 interval pieces and seed block (hand-over arena), which are used in place.  Otherwise (no free
-// hand-over slot, or stage 3) the first iteration is recomputed here.  New samples are solved by seeded Newton from
-// the source centre's seed block, with the cold solver as verified fallback.
+// twk_adaptive.cuh -- a8 + a9: the adaptive contour loop for one source per CTA (refinement stages 2 and 3; see
+// twk_kernels.cuh).  Every iteration adds up to 64 new samples, one thread each; stage 2 runs 64-thread CTAs, stage 3
+// 128-thread CTAs whose extra warps share the O(n) passes over the sorted state.  A stage-2 source normally arrives with
+// its first iteration done: stage 1 handed over its 64 records, 64 interval pieces and seed block (hand-over arena),
+// which are used in place; without a free hand-over slot the first iteration is recomputed here.  A source that fills
+// stage 2's capacity takes its whole state along to stage 3 (carry-over arena) and continues there; without a free
+// carry-over slot stage 3 recomputes it from its first sample.  New samples are solved by seeded Newton from the source
+// centre's seed block, with the cold solver as verified fallback.
 #pragma once
 
 #include "twk_kernels.cuh"

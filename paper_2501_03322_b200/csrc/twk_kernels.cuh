@@ -2,12 +2,13 @@
 // functions a1-a7 in twk_device.cuh / twk_contour.cuh).
 //
 //   fixed_kernel      fixed-sampling mode: theta_j = 2 pi j / N, one CTA per source, records staged in shared memory
-//   adaptive_kernel   the adaptive loop of P:318-326 for one source per 64-thread CTA, entirely on-device:
+//   adaptive_kernel   the adaptive loop of P:318-326 for one source per CTA (64 or 128 threads), entirely on-device:
 //                     64 samples per iteration (one thread each), per-source sorted sample state in shared memory,
 //                     error-weighted inverse-transform sampling, stop rule + cap.
 //                     Refinement stages 2/3 (twk_adaptive.cuh): records in a per-CTA global arena (L2 resident),
 //                     sources taken from the worklist of the previous stage.  Stage 1 (twk_stage1.cuh) is the
 //                     first iteration of every source, everything in shared memory.
+//   coeffs_kernel     parity harness: the Eq.(6) coefficients as the device builds them
 //   dfma_probe_kernel FP64 FMA throughput probe (roofline denominator)
 #pragma once
 
