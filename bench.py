@@ -48,7 +48,10 @@ NCU_METRICS = ("gpu__time_duration.sum,smsp__sass_thread_inst_executed_op_dfma_p
                "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum,smsp__sass_thread_inst_executed_op_dadd_pred_on.sum,"
                "dram__bytes_read.sum,dram__bytes_write.sum,sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active,"
                "smsp__issue_active.avg.pct_of_peak_sustained_active")
-STAGES = ("seeds_kernel", "stage1_kernel", "adaptive_kernel", "adaptive_kernel")      # launch order inside one twk_magnify
+# launch order inside one twk_magnify, and the stage each launch is counted under (stage 1.5, the first refinement iteration in
+# shared memory, belongs to the refinement of stage 2: the library's stage timer brackets the two together)
+STAGES = ("seeds_kernel", "stage1_kernel", "refine1_kernel", "adaptive_kernel", "adaptive_kernel")
+STAGE_KEY = (0, 1, 2, 2, 3)
 
 
 def parse_args():
@@ -230,11 +233,22 @@ def parse_ncu(path):
             dfma = L["smsp__sass_thread_inst_executed_op_dfma_pred_on.sum"]
             dmul = L["smsp__sass_thread_inst_executed_op_dmul_pred_on.sum"]
             dadd = L["smsp__sass_thread_inst_executed_op_dadd_pred_on.sum"]
-            ks[f"stage{s}"] = {"kernel": stage, "dfma": dfma, "dmul": dmul, "dadd": dadd, "flop": 2 * dfma + dmul + dadd,
-                               "dram_bytes": L["dram__bytes_read.sum"] + L["dram__bytes_write.sum"],
-                               "ncu_ms": L["gpu__time_duration.sum"] * 1e-6,
-                               "fp64_pipe_pct": L["sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active"],
-                               "issue_active_pct": L["smsp__issue_active.avg.pct_of_peak_sustained_active"]}
+            one = {"kernel": stage, "dfma": dfma, "dmul": dmul, "dadd": dadd, "flop": 2 * dfma + dmul + dadd,
+                   "dram_bytes": L["dram__bytes_read.sum"] + L["dram__bytes_write.sum"],
+                   "ncu_ms": L["gpu__time_duration.sum"] * 1e-6,
+                   "fp64_pipe_pct": L["sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active"],
+                   "issue_active_pct": L["smsp__issue_active.avg.pct_of_peak_sustained_active"]}
+            key = f"stage{STAGE_KEY[s]}"
+            if key not in ks:
+                ks[key] = one
+            else:   # two launches under one stage: counts and times add, activities are time-weighted
+                o = ks[key]
+                tt = o["ncu_ms"] + one["ncu_ms"]
+                for a in ("fp64_pipe_pct", "issue_active_pct"):
+                    o[a] = (o[a] * o["ncu_ms"] + one[a] * one["ncu_ms"]) / tt if tt > 0 else 0.0
+                for a in ("dfma", "dmul", "dadd", "flop", "dram_bytes", "ncu_ms"):
+                    o[a] += one[a]
+                o["kernel"] = o["kernel"] + " + " + stage
         out["workloads"][name] = ks
     os.makedirs(os.path.dirname(COUNTS), exist_ok=True)
     with open(COUNTS, "w") as f:

@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtwk.so")
 LIB_DEBUG = os.path.join(HERE, "libtwk_debug.so")   # same sources with -DTWK_DEBUG: invariant counters (twk_debug_counters)
 SOURCES = ["twk_api.cu"]
-HEADERS = ["twk_device.cuh", "twk_contour.cuh", "twk_kernels.cuh", "twk_adaptive.cuh", "twk_stage1.cuh"]
+HEADERS = ["twk_device.cuh", "twk_contour.cuh", "twk_kernels.cuh", "twk_adaptive.cuh", "twk_refine1.cuh", "twk_stage1.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
               "-shared", "-cudart", "shared"]
 

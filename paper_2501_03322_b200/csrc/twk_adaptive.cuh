@@ -54,6 +54,8 @@ struct AdaptArgs {
   int subtract_avg_tol;
   int guard;             // L-4 guard: hidden-crossing term in the interval estimates (twk_options.hidden_crossing_guard)
   int final_stage;       // 1: cap reached -> return value + estimate with TWK_ST_CAP; 0: hand to next stage
+  const int32_t* remap;  // stage 2 behind stage 1.5: worklist of ENTRIES (indices into `list` and the hand-over arena) that are
+                         // still to be refined; null: entries 0 .. count - 1 in order
   const int32_t* list;   // worklist of source ids (null: all sources 0..n_sources-1)
   const int* count;      // number of entries of `list` (device; null: n_sources)
   int* cursor;           // dynamic work fetch counter (device, zeroed before launch)
@@ -155,7 +157,8 @@ __global__ void __launch_bounds__(TB, TB == kThreads ? 6 : 2) adaptive_kernel(Ad
     int next_cur = 0;
     if (t == 0) next_cur = atomicAdd(p.cursor, 1);
     // a handed-over source starts from its slot's header; otherwise worklist -> model -> parameters
-    hand = (p.handoff && cur < p.handoff_slots) ? p.handoff + (size_t)cur * kHandDoubles : nullptr;
+    const long long ent = p.remap ? (long long)p.remap[cur] : cur;
+    hand = (p.handoff && ent < p.handoff_slots) ? p.handoff + (size_t)ent * kHandDoubles : nullptr;
     long long src;
     SourceParams S;
     if (hand) {
@@ -170,7 +173,7 @@ __global__ void __launch_bounds__(TB, TB == kThreads ? 6 : 2) adaptive_kernel(Ad
       S.status = (uint32_t)code_of(hd[8]);
       S.valid = true;
     } else {
-      src = p.list ? (long long)p.list[cur] : cur;
+      src = p.list ? (long long)(p.list[ent] & 0x7fffffff) : ent;   // (the sign bit is stage 1's note for stage 1.5)
       S = load_source(p.b, src);
     }
     TWK_CHECK(src >= 0 && src < p.b.n_sources, 4);

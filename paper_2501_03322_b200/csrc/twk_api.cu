@@ -7,6 +7,7 @@
 
 #include "../../include/twk.h"
 #include "twk_adaptive.cuh"
+#include "twk_refine1.cuh"
 #include "twk_stage1.cuh"
 
 namespace {
@@ -55,7 +56,7 @@ size_t handoff_slots(const twk_options& o, size_t max_sources) {
 }
 
 struct Layout {
-  size_t counters, list1, list2, seeds, handoff, carry, arena, total;
+  size_t counters, list1, list1b, list2, seeds, handoff, carry, arena, total;
   size_t slots, carry_slots;
 };
 Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
@@ -65,6 +66,7 @@ Layout make_layout(const twk_options& o, size_t max_sources, int sms) {
   L.slots = handoff_slots(o, max_sources);
   L.counters = off; off += 256;
   L.list1 = off;    off += align256(max_sources * 4);
+  L.list1b = off;   off += align256(max_sources * 4);   // entries stage 1.5 leaves to stage 2
   L.list2 = off;    off += align256(max_sources * 4);
   L.seeds = off;    off += align256(max_sources * twk::kSeedDoubles * 8);
   L.handoff = off;  off += align256(L.slots * twk::kHandDoubles * 8);
@@ -288,7 +290,8 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
   cudaStream_t stream = (cudaStream_t)stream_;
   const Plan& P = ctx->plan;
   int* counters = reinterpret_cast<int*>(ctx->ws + ctx->lay.counters);
-  // counters: [0] cursor1, [1] count1 (stage-2 worklist), [2] cursor2, [3] count2 (stage-3 worklist), [4] cursor3
+  // counters: [0] cursor1, [1] count1 (refinement worklist), [2] cursor2, [3] count2 (stage-3 worklist), [4] cursor3,
+  //           [5] cursor of stage 1.5, [6] count1b (entries stage 1.5 leaves to stage 2)
   TWK_CUDA(cudaMemsetAsync(counters, 0, 64, stream));
   twk::AdaptArgs a{};
   a.b = batch;
@@ -345,13 +348,39 @@ static int magnify_impl(twk_ctx* ctx, const twk::Batch& batch, double rel_tol, d
     ++launches;
     mark();
   }
+  // ---- stage 1.5: the first refinement iteration of the handed-over sources, all in shared memory (twk_refine1.cuh).
+  //      Not with the L-4 guard (its term needs the neighbours' neighbours) and not without hand-over slots.
+  const bool stage15 = P.cap2 >= 2 * twk::kThreads && ctx->lay.slots > 0 && !ctx->opt.hidden_crossing_guard;
+  int32_t* list1b = reinterpret_cast<int32_t*>(ctx->ws + ctx->lay.list1b);
+  if (stage15) {
+    twk::Refine1Args r{};
+    r.b = a.b;
+    r.tol = rel_tol;
+    r.slope_gate2 = a.slope_gate2;
+    r.slope_cos2 = a.slope_cos2;
+    r.subtract_avg_tol = a.subtract_avg_tol;
+    r.list = list1;
+    r.count = counters + 1;
+    r.cursor = counters + 5;
+    r.handoff = handoff;
+    r.handoff_slots = (long long)ctx->lay.slots;
+    r.next_list = list1b;
+    r.next_count = counters + 6;
+    r.out_mu = out_mu;
+    r.out_err = out_err;
+    r.out_nsamples = out_nsamples;
+    r.out_status = out_status;
+    twk::refine1_kernel<<<ctx->sms * kStage2CtasPerSM, twk::kThreads, twk::refine1_smem_bytes(), stream>>>(r);
+    ++launches;
+  }
   if (P.cap2) {
     // ---- stage 2: the worklist stage 1 appended (a9), first iteration handed over -------------------------------------
     twk::AdaptArgs a2 = a;
     a2.cap = P.cap2;
     a2.final_stage = P.cap3 ? 0 : 1;
     a2.list = list1;
-    a2.count = counters + 1;
+    a2.count = stage15 ? counters + 6 : counters + 1;
+    a2.remap = stage15 ? list1b : nullptr;
     a2.cursor = counters + 2;
     a2.next_list = list2;
     a2.next_count = counters + 3;

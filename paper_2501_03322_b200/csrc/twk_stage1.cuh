@@ -233,14 +233,27 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
       const bool pend = finite && !(E <= p.tol * fabs(A)) && !p.final_stage;   // stop rule P:272
       if (pend) {
         // a9: append to the refinement worklist; hand the first-iteration state over when a slot is free
+        // Is ONE more iteration (64 samples where the error is) likely to finish this source?  If the error sits in
+        // N_eff = E^2 / sum e_i^2 intervals, each gets ~64 / N_eff new samples and its error falls by about the square of
+        // that: predicted E / (1 + 64 sum e_i^2 / E^2)^2.  A source whose prediction is still above 1.5 tolerances (error
+        // spread evenly at a tight tolerance) is marked (sign bit of its worklist entry): stage 1.5 leaves it to stage 2.
+        double q2 = P.err * P.err;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) q2 += __shfl_xor_sync(0xffffffffu, q2, o);
+        double* sq = scratch + parity * 4;   // (the half of the double buffer the NEXT reduction will use: free now)
+        if ((t & 31) == 0) sq[warp] = q2;
         if (t == 0) {
           const int slot = atomicAdd(p.list_count, 1);
           TWK_CHECK(slot >= 0 && slot < n, 4);
-          p.list[slot] = (int32_t)(base + i);
           iscr[3] = slot;
         }
         __syncthreads();
         const long long slot = iscr[3];
+        if (t == 0) {
+          const double S2 = sq[0] + sq[1], E2 = E * E, den = E2 + 64.0 * S2;
+          const bool spread = E * E2 * E2 > 1.5 * p.tol * fabs(A) * den * den;   // E / (1 + 64 S2 / E^2)^2 > 1.5 tol |A|
+          p.list[slot] = (int32_t)(base + i) | (spread ? (int32_t)0x80000000 : 0);
+        }
         if (slot < p.handoff_slots) {
           double* h = p.handoff + (size_t)slot * kHandDoubles;
 #pragma unroll

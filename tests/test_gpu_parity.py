@@ -298,8 +298,9 @@ def test_point_source_tests_full_size_against_contour(ctx_ps):
 
 
 def test_handover_and_recompute_paths_agree():
-    """Stage 1 hands the first iteration of an unfinished source to stage 2 through the hand-over arena; without a
-    free slot stage 2 recomputes it.  Same arithmetic either way (up to the compiler's contraction choices in the
+    """Stage 1 hands the first iteration of an unfinished source on through the hand-over arena: stage 1.5 does the first
+    refinement iteration from it in shared memory and finishes most sources, stage 2 continues the rest from the same
+    slot; without a free slot stage 2 recomputes the source from its first sample.  Same arithmetic either way (up to the compiler's contraction choices in the
     two kernels): identical sample counts and status, mu to rounding amplified by the sampler."""
     import paper_2501_03322_b200 as P
     full = W.config4()
@@ -312,6 +313,9 @@ def test_handover_and_recompute_paths_agree():
         res.append(c.magnify_workload(wl, 1e-5))
         st = c.twk_last_stats()
         assert st["n_stage2"] > 1000           # most of the band refines
+        # with hand-over slots the first refinement iteration has a kernel of its own (stage 1.5, shared memory only);
+        # entries beyond the slots pass through it untouched; without slots it is not launched
+        assert st["n_launches"] == (4 if slots == 0 else 5)
         c.close()
     for r in res[1:]:
         # (the recomputed first iteration takes its interval widths from theta_{i+1} - theta_i, the handed-over one from
