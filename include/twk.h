@@ -201,12 +201,14 @@ int twk_last_stage_ms(twk_ctx* ctx, float* ms4);
 int twk_fp64_peak_probe(int iters, double* out_tflops);
 
 /* Debug build only (libtwk_debug.so, compiled with -DTWK_DEBUG; twk_version() says so): the kernels count violations of
- * their own invariants instead of trapping -- out8 = {record id out of range, sample angles not strictly increasing,
- * sorted list not a permutation of the sample ids, two writers to one record in one re-judging phase, worklist / hand-over
- * slot out of range, new angle outside its interval, sources checked, iterations checked}.  Synchronises the device;
+ * their own invariants instead of trapping -- out12 (12 values, caller-owned host memory) = {record id out of range, sample
+ * angles not strictly increasing, sorted list not a permutation of the sample ids, two writers to one record in one
+ * re-judging phase, worklist / hand-over slot out of range, new angle outside its interval, sources checked, iterations
+ * checked, and four event counts of stage 1.5: entries taken up, entries whose new samples were solved, sources finished
+ * there, entries passed on unread}.  Synchronises the device;
  * reset != 0 clears the counters.  Returns TWK_EINVAL in the release build.  Stands in for compute-sanitizer, which this
  * pool does not offer. */
-int twk_debug_counters(uint32_t* out8, int reset);
+int twk_debug_counters(uint32_t* out12, int reset);
 
 const char* twk_strerror(int code);
 const char* twk_version(void);

@@ -101,7 +101,7 @@ def twk_version() -> str:
 
 def twk_debug_counters(reset: bool = False):
     """Invariant-violation counters of the debug build (raises TwkError on the release build)."""
-    out = (C.c_uint32 * 8)()
+    out = (C.c_uint32 * 12)()
     _check(lib().twk_debug_counters(out, 1 if reset else 0), "twk_debug_counters")
     return [int(x) for x in out]
 

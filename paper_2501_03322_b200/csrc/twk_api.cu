@@ -639,18 +639,18 @@ int twk_fp64_peak_probe(int iters, double* out_tflops) {
   return TWK_OK;
 }
 
-int twk_debug_counters(uint32_t* out8, int reset) {
+int twk_debug_counters(uint32_t* out12, int reset) {
 #ifdef TWK_DEBUG
-  if (!out8) return TWK_EINVAL;
+  if (!out12) return TWK_EINVAL;
   TWK_CUDA(cudaDeviceSynchronize());
-  TWK_CUDA(cudaMemcpyFromSymbol(out8, twk::g_twk_debug, 8 * sizeof(uint32_t)));
+  TWK_CUDA(cudaMemcpyFromSymbol(out12, twk::g_twk_debug, 12 * sizeof(uint32_t)));
   if (reset) {
-    uint32_t z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    uint32_t z[12] = {0};
     TWK_CUDA(cudaMemcpyToSymbol(twk::g_twk_debug, z, sizeof(z)));
   }
   return TWK_OK;
 #else
-  (void)out8;
+  (void)out12;
   (void)reset;
   return TWK_EINVAL;   // not a debug build
 #endif

@@ -26,9 +26,12 @@ namespace twk {
 //   [2] sorted list is not a permutation of the ids  [3] a record re-judged by two threads in one phase
 //   [4] worklist / hand-over slot out of range       [5] a new angle outside the interval that owns its quantile
 //   [6] sources checked by the refinement stages     [7] iterations checked
+// and four plain event counts of stage 1.5 (twk_refine1.cuh):
+//   [8] entries taken up                              [9] of those, entries whose new samples were solved
+//   [10] of those, sources finished there             [11] entries passed on unread (no hand-over slot / stage 1's mark)
 // ------------------------------------------------------------------------------------------------------------
 #ifdef TWK_DEBUG
-__device__ unsigned g_twk_debug[8];
+__device__ unsigned g_twk_debug[12];
 __device__ unsigned g_twk_stamp[2048 * 64];   // one bit per record of every CTA's arena slot (<= 2048 CTAs x 4096 records)
 #define TWK_CHECK(cond, which)                            \
   do {                                                    \

@@ -96,6 +96,10 @@ __global__ void __launch_bounds__(kThreads, 6) refine1_kernel(Refine1Args p) {
       off = __shfl_sync(0xffffffffu, off, 0);
       if (skip) p.next_list[off + __popc(skips & ((1u << lane) - 1u))] = (int32_t)e;
       if (lane == 0) iscr[5] = (int)(valids & ~skips);
+#ifdef TWK_DEBUG
+      if (skip) TWK_DEBUG_COUNT(11);
+      if (skip) TWK_CHECK(off + __popc(skips & ((1u << lane) - 1u)) < total, 4);
+#endif
     }
     __syncthreads();
     const unsigned todo = (unsigned)iscr[5];
@@ -105,6 +109,8 @@ __global__ void __launch_bounds__(kThreads, 6) refine1_kernel(Refine1Args p) {
     const long long cur = chunk + b;
     bool pass_on = false;   // (uniform) leave this entry to stage 2 after all
     const double* hand = p.handoff + (size_t)cur * kHandDoubles;
+    TWK_CHECK(cur >= 0 && cur < total && cur < p.handoff_slots, 4);
+    if (t == 0) TWK_DEBUG_COUNT(8);
     long long src = 0;
     SourceParams S;
     S.valid = false;
@@ -243,6 +249,13 @@ __global__ void __launch_bounds__(kThreads, 6) refine1_kernel(Refine1Args p) {
         }
         __syncthreads();
         if (m == 0) pass_on = true;   // (stage 2 comes to the same conclusion and sends the source on)
+#ifdef TWK_DEBUG
+        if (t < m) {   // a new angle lies strictly inside the interval that owns its quantile; owners do not decrease
+          const int i = cint[t];
+          TWK_CHECK(i >= 0 && i < n && cth[t] > theta[i] && cth[t] < ((i + 1 < n) ? theta[i + 1] : kTwoPi), 5);
+          TWK_CHECK(t == 0 || cint[t - 1] <= i, 5);
+        }
+#endif
         }
       }
     }
@@ -280,6 +293,20 @@ __global__ void __launch_bounds__(kThreads, 6) refine1_kernel(Refine1Args p) {
       n_new = n + m;
       cp_async_wait_all();   // this thread's chunks of tile A have landed ...
       __syncthreads();       // ... and so have everybody else's; the new records are complete
+#ifdef TWK_DEBUG
+      for (int i = t; i < n_new; i += kThreads) {
+        TWK_CHECK(ids[i] < n_new, 0);
+        if (i + 1 < n_new) TWK_CHECK(theta[i] < theta[i + 1], 1);
+        int seen = 0;   // record id i sits at exactly one sorted position
+        for (int j = 0; j < n_new; ++j) seen += (ids[j] == i);
+        TWK_CHECK(seen == 1, 2);
+      }
+      if (t == 0) {
+        TWK_DEBUG_COUNT(6);
+        TWK_DEBUG_COUNT(7);
+        TWK_DEBUG_COUNT(9);
+      }
+#endif
       // ---- re-evaluate only the intervals that changed ------------------------------------------------------------
       if (t < m) {
         const bool last_in_group = (t == m - 1) || (cint[t + 1] != cint[t]);
@@ -327,8 +354,11 @@ __global__ void __launch_bounds__(kThreads, 6) refine1_kernel(Refine1Args p) {
         if (p.out_err) p.out_err[src] = E * rcp(fabs(A));
         if (p.out_nsamples) p.out_nsamples[src] = n_new;
         if (p.out_status) p.out_status[src] = status;
+        TWK_DEBUG_COUNT(10);
       } else {
-        p.next_list[atomicAdd(p.next_count, 1)] = (int32_t)cur;   // stage 2 takes it from its hand-over slot
+        const int at = atomicAdd(p.next_count, 1);
+        TWK_CHECK(at >= 0 && at < total, 4);
+        p.next_list[at] = (int32_t)cur;   // stage 2 takes it from its hand-over slot
       }
     }
     }   // entries of the chunk

@@ -50,6 +50,9 @@ def test_debug_build_invariants_hold():
     c = json.loads(out.stdout.strip().splitlines()[-1])
     assert c[:6] == [0, 0, 0, 0, 0, 0], c          # no violation of any invariant
     assert c[6] > 10000 and c[7] > 20000, c         # ... and the checks ran: sources and iterations checked
+    # stage 1.5 took part: entries taken up >= entries solved >= sources finished there > 0; some were passed on unread
+    # (the handoff_slots = 0 contexts do not launch it)
+    assert c[8] >= c[9] >= c[10] > 1000 and c[11] > 0, c
 
 
 def test_release_build_has_no_debug_counters():
