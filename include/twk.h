@@ -59,8 +59,9 @@ typedef struct {
   int max_samples;      /* sample cap per source, default 4096; 64 <= max_samples <= 4096                  */
   int subtract_avg_tol; /* 1 = subtract the average tolerance from every interval error before sampling */
   int64_t handoff_slots; /* slots of the hand-over arena through which the first iteration (64 records, interval     */
-                        /* pieces, seeds; 14,720 B per slot) of an unfinished source passes to the refinement stage  */
-                        /* instead of being recomputed there.  -1 = default min(max_sources, 524288); 0 = none.      */
+                        /* pieces, seeds; 14,720 B per slot) of an unfinished source passes to the refinement stages */
+                        /* (the first refinement iteration in a kernel of its own, all in shared memory, then the     */
+                        /* 512-sample stage) instead of being recomputed there.  -1 = default min(max_sources, 524288); 0 = none.      */
                         /* Sources beyond the slots are still refined (their first iteration is recomputed).  A context */
                         /* with slots also gets 1024 carry-over slots (120 KB each) through which a source that fills */
                         /* the 512-sample refinement stage takes its whole state to the 4096-sample stage; with 0     */
@@ -184,14 +185,17 @@ int twk_magnify_host(twk_ctx* ctx, size_t n_models, const double* s, const doubl
                      size_t n_sources, const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu,
                      double* out_err, int32_t* out_nsamples, uint32_t* out_status, void* stream);
 
-/* Diagnostics of the last twk_magnify on this context (synchronises `stream`): number of sources handed to the
- * refinement stages 2 and 3, and the number of kernels the call launched.  Any pointer may be NULL. */
+/* Diagnostics of the last twk_magnify on this context (synchronises `stream`): number of sources the first iteration
+ * left unfinished (*n_stage2: the worklist of the refinement stages 1.5 and 2), number that filled the 512-sample stage
+ * and went on to the last one (*n_stage3), and the number of kernels the call launched (5 with hand-over slots: centre
+ * solves, first iteration, first refinement iteration in shared memory, 512-sample stage, max_samples stage; 4 without:
+ * the third is then not launched).  Any pointer may be NULL. */
 int twk_last_stats(twk_ctx* ctx, int64_t* n_stage2, int64_t* n_stage3, int* n_launches, void* stream);
 
 /* Per-stage device timing of twk_magnify for measurement: when enabled, CUDA events are recorded on the call's
  * stream around each stage.  twk_last_stage_ms waits for the last recorded event and writes the durations (ms)
- * of {stage-0 (centre solves), stage-1, stage-2, stage-3 kernel} of the last twk_magnify on this context (0 for
- * absent stages) into ms4[4]. */
+ * of {stage-0 (centre solves), stage-1, stage-1.5 + stage-2, stage-3 kernel} of the last twk_magnify on this context
+ * (0 for absent stages) into ms4[4]. */
 int twk_enable_stage_timing(twk_ctx* ctx, int on);
 int twk_last_stage_ms(twk_ctx* ctx, float* ms4);
 

@@ -8,6 +8,9 @@
 //                     Refinement stages 2/3 (twk_adaptive.cuh): records in a per-CTA global arena (L2 resident),
 //                     sources taken from the worklist of the previous stage.  Stage 1 (twk_stage1.cuh) is the
 //                     first iteration of every source, everything in shared memory.
+//   refine1_kernel    stage 1.5 (twk_refine1.cuh): the first refinement iteration (64 -> up to 128 samples) of the sources
+//                     stage 1 handed over, old and new records in two shared-memory tiles; what it cannot finish is left
+//                     to stage 2 untouched.
 //   coeffs_kernel     parity harness: the Eq.(6) coefficients as the device builds them
 //   dfma_probe_kernel FP64 FMA throughput probe (roofline denominator)
 #pragma once
