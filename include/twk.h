@@ -36,6 +36,7 @@ extern "C" {
 #define TWK_EINVAL (-1) /* null required pointer, N < 4, rel_tol <= 0, bad options, n_sources > max_sources */
 #define TWK_ENOMEM (-2) /* workspace allocation failed */
 #define TWK_ECUDA (-3)  /* a CUDA runtime call failed; twk_strerror gives the CUDA text of the last one */
+#define TWK_ELIMIT (-4) /* twk_magnify_static: n_sources > TWK_STATIC_MAX_SOURCES (its scratch has a fixed size) */
 
 /* per-source status bits (out_status) */
 #define TWK_ST_CONVERGED 1u  /* error estimate <= rel_tol * |A|                                       */
@@ -184,6 +185,27 @@ int twk_coeffs_eq6(twk_ctx* ctx, size_t n_models, const double* s, const double*
 int twk_magnify_host(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
                      size_t n_sources, const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu,
                      double* out_err, int32_t* out_nsamples, uint32_t* out_status, void* stream);
+
+/* The adaptive mode for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): twk_magnify without a context.  Same kernels, same arguments and results as twk_magnify on a
+ * context created with default options and handoff_slots = 0 (every refinement starts again from the source's first
+ * sample; results agree with the default context's within the tolerance, most of them bit for bit); all pointers DEVICE,
+ * asynchronous on `stream`.  The call and everything under it calls no cudaMalloc, cudaFree or allocating library routine:
+ * its workspace (counters, worklists, seed blocks, the refinement stages' record arena) is a fixed array in the library's
+ * device image, TWK_STATIC_SCRATCH_BYTES per GPU, held by every GPU that loads the library until the process exits.
+ *   - Limit: n_sources <= TWK_STATIC_MAX_SOURCES, else TWK_ELIMIT (nothing is launched); split larger batches or use a
+ *     context.  The refinement stages run on 128 and 16 CTAs here (their record arena is what the scratch mostly is),
+ *     so a batch in which most sources refine is slower than on a context.
+ *   - Every call on a device shares the one array, which keeps the previous call's contents.  The call clears the work
+ *     counters itself (on `stream`); everything else is written before it is read.  Calls that OVERLAP on the GPU (two
+ *     streams, two host threads) race on it: keep calls on one device in stream order.
+ *   - The first call on each device looks the array's device address up (cudaGetSymbolAddress, with that device current)
+ *     and sets a function attribute; make that call outside a graph capture. */
+#define TWK_STATIC_MAX_SOURCES 16384
+#define TWK_STATIC_SCRATCH_BYTES (18u << 20) /* 18 MiB: 256 B counters + 3 x 64 KiB lists + 3.9 MiB seed blocks + 13 MiB arena */
+int twk_magnify_static(size_t n_models, const double* s, const double* q, const double* rho, size_t n_sources,
+                       const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu, double* out_err,
+                       int32_t* out_nsamples, uint32_t* out_status, void* stream);
 
 /* Diagnostics of the last twk_magnify on this context (synchronises `stream`): number of sources the first iteration
  * left unfinished (*n_stage2: the worklist of the refinement stages 1.5 and 2), number that filled the 512-sample stage

@@ -19,7 +19,7 @@ TWK_ST_CONVERGED, TWK_ST_CAP, TWK_ST_REPAIRED, TWK_ST_DOMAIN, TWK_ST_NUMERIC, TW
 
 SYMBOLS = ["twk_default_options", "twk_create", "twk_destroy", "twk_workspace_bytes", "twk_magnify", "twk_magnify_lightcurve", "twk_magnify_lightcurve_orbital",
            "twk_images_fixed", "twk_images_fixed_seeded", "twk_stage1_records",
-           "twk_coeffs_eq6", "twk_magnify_host", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_debug_counters", "twk_strerror", "twk_version"]
+           "twk_coeffs_eq6", "twk_magnify_host", "twk_magnify_static", "twk_last_stats", "twk_enable_stage_timing", "twk_last_stage_ms", "twk_fp64_peak_probe", "twk_debug_counters", "twk_strerror", "twk_version"]
 
 
 class TwkError(RuntimeError):
@@ -54,6 +54,7 @@ def lib():
         L.twk_magnify_lightcurve.argtypes = [vp, sz, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
         L.twk_magnify_lightcurve_orbital.argtypes = [vp, sz, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
         L.twk_magnify_host.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
+        L.twk_magnify_static.argtypes = [sz, vp, vp, vp, sz, vp, vp, dbl, vp, vp, vp, vp, vp]
         L.twk_images_fixed.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, vp]
         L.twk_images_fixed_seeded.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
         L.twk_stage1_records.argtypes = [vp, sz, vp, vp, vp, sz, vp, vp, vp, vp, vp]
@@ -104,6 +105,24 @@ def twk_debug_counters(reset: bool = False):
     out = (C.c_uint32 * 12)()
     _check(lib().twk_debug_counters(out, 1 if reset else 0), "twk_debug_counters")
     return [int(x) for x in out]
+
+
+TWK_STATIC_MAX_SOURCES = 16384   # include/twk.h
+TWK_ELIMIT = -4
+
+
+def twk_magnify_static(s, q, rho, zeta, out_mu, model_id=None, rel_tol=1e-4, out_err=None, out_nsamples=None, out_status=None,
+                       stream=None):
+    """twk_magnify without a context and without any allocation: the workspace is a fixed array inside the library
+    (include/twk.h).  All tensors CUDA and caller-owned, outputs included (this wrapper allocates nothing either);
+    at most TWK_STATIC_MAX_SOURCES sources; calls on one device must not overlap.  Returns the library's code
+    (0, or TWK_ELIMIT for a batch beyond the limit); other errors raise."""
+    n = int(zeta.shape[0])
+    rc = lib().twk_magnify_static(int(s.shape[0]), _ptr(s), _ptr(q), _ptr(rho), n, _ptr(model_id), _ptr(zeta), float(rel_tol),
+                                  _ptr(out_mu), _ptr(out_err), _ptr(out_nsamples), _ptr(out_status), _stream_ptr(stream))
+    if rc != TWK_ELIMIT:
+        _check(rc, "twk_magnify_static")
+    return rc
 
 
 def twk_fp64_peak_probe(iters: int = 1 << 16) -> float:

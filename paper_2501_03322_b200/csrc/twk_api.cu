@@ -3,6 +3,7 @@
 
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "../../include/twk.h"
@@ -639,6 +640,108 @@ int twk_fp64_peak_probe(int iters, double* out_tflops) {
   return TWK_OK;
 }
 
+// ---- twk_magnify_static: the adaptive path with NO allocation ------------------------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops, harnesses that forbid it): the
+// workspace of the same kernels -- counters, worklists, seed blocks, the refinement stages' record arena -- lives in a
+// file-scope __device__ array instead of a context's cudaMalloc'ed block.  Every GPU that loads the library holds the
+// array (TWK_STATIC_SCRATCH_BYTES) until the process exits; every call on a device shares it.
+namespace {
+constexpr size_t kStaticMaxSources = TWK_STATIC_MAX_SOURCES;
+constexpr int kStaticGrid2 = 128, kStaticGrid3 = 16;   // CTAs of the two refinement stages (each owns a slice of the arena)
+constexpr int kStaticMaxDevices = 64;
+constexpr size_t static_align256(size_t x) { return (x + 255) & ~size_t(255); }
+constexpr size_t kStaticArenaRecords =
+    (size_t)kStaticGrid2 * kStage2Cap > (size_t)kStaticGrid3 * 4096 ? (size_t)kStaticGrid2 * kStage2Cap : (size_t)kStaticGrid3 * 4096;
+// counters | list1 | list1b | list2 | seed blocks | record arena (no hand-over and no carry-over slots: the lean layout)
+constexpr size_t kStaticNeed = 256 + 3 * static_align256(kStaticMaxSources * 4) +
+                               static_align256(kStaticMaxSources * twk::kSeedDoubles * 8) +
+                               static_align256(kStaticArenaRecords * twk::kRecDoubles * 8);
+static_assert(kStaticNeed <= TWK_STATIC_SCRATCH_BYTES, "TWK_STATIC_SCRATCH_BYTES too small for TWK_STATIC_MAX_SOURCES");
+}  // namespace
+
+// In host code this name is only a handle for cudaGetSymbolAddress: it is NOT a device address.
+static __device__ __align__(256) unsigned char g_twk_static_scratch[TWK_STATIC_SCRATCH_BYTES];
+
+namespace {
+struct StaticSlot {
+  bool ready;
+  twk_ctx ctx;
+};
+StaticSlot g_static[kStaticMaxDevices];   // one per device, host memory of the library image (no allocation)
+std::mutex g_static_mutex;
+
+// Set-up, once per device, with that device current: the array's device address, the plan and the layout.
+int static_context(twk_ctx** out) {
+  int dev = 0;
+  TWK_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kStaticMaxDevices) return TWK_EINVAL;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticSlot& S = g_static[dev];
+  if (!S.ready) {
+    int sms = 0;
+    TWK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    void* base = nullptr;
+    TWK_CUDA(cudaGetSymbolAddress(&base, g_twk_static_scratch));
+    if (!base) return TWK_ECUDA;
+    twk_ctx& c = S.ctx;
+    twk_default_options(&c.opt);
+    c.opt.handoff_slots = 0;
+    c.max_sources = kStaticMaxSources;
+    c.sms = sms;
+    c.plan = make_plan(c.opt, sms);
+    c.plan.grid2 = kStaticGrid2;   // any grid works: the CTAs are persistent and fetch their sources from a cursor
+    c.plan.grid3 = kStaticGrid3;
+    c.plan.arena_doubles = kStaticArenaRecords * twk::kRecDoubles;
+    Layout L{};
+    size_t off = 0;
+    L.counters = off; off += 256;
+    L.list1 = off;    off += align256(kStaticMaxSources * 4);
+    L.list1b = off;   off += align256(kStaticMaxSources * 4);
+    L.list2 = off;    off += align256(kStaticMaxSources * 4);
+    L.seeds = off;    off += align256(kStaticMaxSources * twk::kSeedDoubles * 8);
+    L.handoff = off;
+    L.carry = off;
+    L.arena = off;    off += align256(c.plan.arena_doubles * 8);
+    L.total = off;
+    L.slots = 0;
+    L.carry_slots = 0;
+    if (L.total > sizeof(g_twk_static_scratch)) return TWK_EINVAL;   // (the static_assert above says it cannot be)
+    c.lay = L;
+    c.ws = static_cast<char*>(base);
+    c.stage = nullptr;
+    c.stage_bytes = 0;
+    c.last_launches = 0;
+    c.timing = 0;
+    c.ev_used = 0;
+    for (int i = 0; i < 5; ++i) c.ev[i] = nullptr;
+    // the large dynamic shared memory of the last stage is a per-device function attribute (no allocation)
+    TWK_CUDA(cudaFuncSetAttribute(twk::adaptive_kernel<false, false, false, kStage3Threads>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)twk::adaptive_smem_bytes(4096, false, false, kStage3Threads)));
+    S.ready = true;
+  }
+  *out = &S.ctx;
+  return TWK_OK;
+}
+}  // namespace
+
+int twk_magnify_static(size_t n_models, const double* s, const double* q, const double* rho, size_t n_sources,
+                       const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu, double* out_err,
+                       int32_t* out_nsamples, uint32_t* out_status, void* stream_) {
+  if (n_sources > kStaticMaxSources) return TWK_ELIMIT;
+  if (n_sources == 0) return TWK_OK;
+  twk_ctx* ctx = nullptr;
+  const int r0 = static_context(&ctx);
+  if (r0 != TWK_OK) return r0;
+  const int rc = check_batch(ctx, n_models, s, q, rho, n_sources, model_id, zeta);
+  if (rc != TWK_OK) return rc;
+  if (!out_mu || !(rel_tol > 0.0)) return TWK_EINVAL;
+  const twk::Batch b{s, q, rho, model_id, zeta, (long long)n_models, (long long)n_sources, ctx->opt.frame,
+                     nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  // (the call clears the 64 bytes of counters on the stream; every other part of the scratch is written before it is read)
+  return magnify_impl(ctx, b, rel_tol, out_mu, out_err, out_nsamples, out_status, stream_);
+}
+
 int twk_debug_counters(uint32_t* out12, int reset) {
 #ifdef TWK_DEBUG
   if (!out12) return TWK_EINVAL;
@@ -662,6 +765,7 @@ const char* twk_strerror(int code) {
     case TWK_EINVAL: return "invalid argument";
     case TWK_ENOMEM: return "out of device memory for the workspace";
     case TWK_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA runtime error";
+    case TWK_ELIMIT: return "batch larger than TWK_STATIC_MAX_SOURCES, the limit of twk_magnify_static's fixed scratch (use a context)";
     default: return "unknown twk error code";
   }
 }
