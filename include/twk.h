@@ -181,7 +181,11 @@ int twk_coeffs_eq6(twk_ctx* ctx, size_t n_models, const double* s, const double*
 
 /* End-to-end convenience with HOST buffers (same meaning as twk_magnify): copies the inputs host->device into the
  * context's staging area, runs twk_magnify on `stream`, copies the outputs device->host and synchronises the
- * stream before returning.  Optional outputs may be NULL. */
+ * stream before returning.  Optional outputs may be NULL.  A batch of 2,097,152 sources or more goes through in chunks
+ * of about that size (the sources are independent): the kernels of every chunk run on `stream` in order, the
+ * copies of the neighbouring chunks run beside them on two copy streams the context creates on first use (pinned host
+ * buffers make them asynchronous; pageable ones work, without the overlap).  Per-source results do not depend on the
+ * chunking; twk_last_stats / twk_last_stage_ms then describe the last chunk (n_launches: all of them). */
 int twk_magnify_host(twk_ctx* ctx, size_t n_models, const double* s, const double* q, const double* rho,
                      size_t n_sources, const int32_t* model_id, const double* zeta, double rel_tol, double* out_mu,
                      double* out_err, int32_t* out_nsamples, uint32_t* out_status, void* stream);

@@ -131,6 +131,15 @@ void launch_stage1(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t
   else twk::stage1_kernel<false><<<grid, twk::kThreads, smem, stream>>>(a);
 }
 
+constexpr int kHostChunksMax = 8;
+// twk_magnify_host splits batches of at least kHostSplitMin sources into chunks of about kHostChunk (measured on config 3,
+// 4,096,000 sources, pinned host buffers: see DESIGN.md section 6)
+constexpr size_t kHostSplitMin = (size_t)1 << 21;
+#ifndef TWK_HOST_CHUNK
+#define TWK_HOST_CHUNK ((size_t)1 << 21)
+#endif
+constexpr size_t kHostChunk = TWK_HOST_CHUNK;
+
 struct twk_ctx {
   twk_options opt;
   size_t max_sources;
@@ -141,6 +150,10 @@ struct twk_ctx {
   // host staging for twk_magnify_host (allocated on first use)
   char* stage;
   size_t stage_bytes;
+  // twk_magnify_host on a large batch: copy streams and events that overlap the transfers of one chunk with the kernels
+  // of another (created on first use)
+  cudaStream_t copy_in, copy_out;
+  cudaEvent_t ev_in[kHostChunksMax], ev_done[kHostChunksMax], ev_first, ev_last;
   int last_launches;
   int timing;            // record CUDA events around every stage (twk_enable_stage_timing)
   cudaEvent_t ev[5];     // start, after stage 0, after stage 1, after stage 2, after stage 3
@@ -197,6 +210,9 @@ int twk_create(twk_ctx** ctx, const twk_options* opt, size_t max_sources) {
   c->ws = nullptr;
   c->stage = nullptr;
   c->stage_bytes = 0;
+  c->copy_in = c->copy_out = nullptr;
+  c->ev_first = c->ev_last = nullptr;
+  for (int i = 0; i < kHostChunksMax; ++i) c->ev_in[i] = c->ev_done[i] = nullptr;
   c->last_launches = 0;
   c->timing = 0;
   c->ev_used = 0;
@@ -229,6 +245,14 @@ int twk_destroy(twk_ctx* ctx) {
   if (ctx->stage) cudaFree(ctx->stage);
   for (int i = 0; i < 5; ++i)
     if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+  for (int i = 0; i < kHostChunksMax; ++i) {
+    if (ctx->ev_in[i]) cudaEventDestroy(ctx->ev_in[i]);
+    if (ctx->ev_done[i]) cudaEventDestroy(ctx->ev_done[i]);
+  }
+  if (ctx->ev_first) cudaEventDestroy(ctx->ev_first);
+  if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);
+  if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
+  if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
   delete ctx;
   return TWK_OK;
 }
@@ -557,15 +581,82 @@ int twk_magnify_host(twk_ctx* ctx, size_t n_models, const double* s, const doubl
   TWK_CUDA(cudaMemcpyAsync(d_s, s, n_models * 8, cudaMemcpyHostToDevice, stream));
   TWK_CUDA(cudaMemcpyAsync(d_q, q, n_models * 8, cudaMemcpyHostToDevice, stream));
   TWK_CUDA(cudaMemcpyAsync(d_rho, rho, n_models * 8, cudaMemcpyHostToDevice, stream));
-  if (model_id) TWK_CUDA(cudaMemcpyAsync(d_mid, model_id, n_sources * 4, cudaMemcpyHostToDevice, stream));
-  TWK_CUDA(cudaMemcpyAsync(d_zeta, zeta, n_sources * 16, cudaMemcpyHostToDevice, stream));
-  const int r2 = twk_magnify(ctx, n_models, d_s, d_q, d_rho, n_sources, model_id ? d_mid : nullptr, d_zeta, rel_tol, d_mu,
-                             out_err ? d_err : nullptr, out_nsamples ? d_ns : nullptr, out_status ? d_st : nullptr, stream_);
-  if (r2 != TWK_OK) return r2;
-  TWK_CUDA(cudaMemcpyAsync(out_mu, d_mu, n_sources * 8, cudaMemcpyDeviceToHost, stream));
-  if (out_err) TWK_CUDA(cudaMemcpyAsync(out_err, d_err, n_sources * 8, cudaMemcpyDeviceToHost, stream));
-  if (out_nsamples) TWK_CUDA(cudaMemcpyAsync(out_nsamples, d_ns, n_sources * 4, cudaMemcpyDeviceToHost, stream));
-  if (out_status) TWK_CUDA(cudaMemcpyAsync(out_status, d_st, n_sources * 4, cudaMemcpyDeviceToHost, stream));
+  if (n_sources < kHostSplitMin) {   // one piece, everything in stream order
+    if (model_id) TWK_CUDA(cudaMemcpyAsync(d_mid, model_id, n_sources * 4, cudaMemcpyHostToDevice, stream));
+    TWK_CUDA(cudaMemcpyAsync(d_zeta, zeta, n_sources * 16, cudaMemcpyHostToDevice, stream));
+    const int r2 = twk_magnify(ctx, n_models, d_s, d_q, d_rho, n_sources, model_id ? d_mid : nullptr, d_zeta, rel_tol, d_mu,
+                               out_err ? d_err : nullptr, out_nsamples ? d_ns : nullptr, out_status ? d_st : nullptr, stream_);
+    if (r2 != TWK_OK) return r2;
+    TWK_CUDA(cudaMemcpyAsync(out_mu, d_mu, n_sources * 8, cudaMemcpyDeviceToHost, stream));
+    if (out_err) TWK_CUDA(cudaMemcpyAsync(out_err, d_err, n_sources * 8, cudaMemcpyDeviceToHost, stream));
+    if (out_nsamples) TWK_CUDA(cudaMemcpyAsync(out_nsamples, d_ns, n_sources * 4, cudaMemcpyDeviceToHost, stream));
+    if (out_status) TWK_CUDA(cudaMemcpyAsync(out_status, d_st, n_sources * 4, cudaMemcpyDeviceToHost, stream));
+    TWK_CUDA(cudaStreamSynchronize(stream));
+    return TWK_OK;
+  }
+  // A large batch goes through in chunks: the sources are independent, so the host->device copy of chunk c + 1 and
+  // the device->host copy of chunk c - 1 run on two copy streams while the kernels of chunk c run on `stream`.  The chunks
+  // share the context's workspace and are serialised on `stream`; only the transfers overlap.
+  if (!ctx->copy_in) {
+    TWK_CUDA(cudaStreamCreateWithFlags(&ctx->copy_in, cudaStreamNonBlocking));
+    TWK_CUDA(cudaStreamCreateWithFlags(&ctx->copy_out, cudaStreamNonBlocking));
+    TWK_CUDA(cudaEventCreateWithFlags(&ctx->ev_first, cudaEventDisableTiming));
+    TWK_CUDA(cudaEventCreateWithFlags(&ctx->ev_last, cudaEventDisableTiming));
+    for (int i = 0; i < kHostChunksMax; ++i) {
+      TWK_CUDA(cudaEventCreateWithFlags(&ctx->ev_in[i], cudaEventDisableTiming));
+      TWK_CUDA(cudaEventCreateWithFlags(&ctx->ev_done[i], cudaEventDisableTiming));
+    }
+  }
+  // chunk boundaries: chunks of `per` sources, except that the first one is half that size -- its host->device copy and
+  // the last chunk's device->host copy are the transfers nothing overlaps
+  size_t per = kHostChunk, lim = (n_sources + kHostChunksMax - 2) / (kHostChunksMax - 1);
+  if (per < lim) per = lim;
+  per = (per + 8191) / 8192 * 8192;
+  size_t bound[kHostChunksMax + 1];
+  int n_chunks = 0;
+  bound[0] = 0;
+  for (size_t off = 0; off < n_sources;) {
+    const size_t want = (n_chunks == 0) ? per / 2 : per;
+    off = (n_sources - off <= want || n_chunks == kHostChunksMax - 1) ? n_sources : off + want;
+    bound[++n_chunks] = off;
+  }
+  const bool identity = !model_id && n_models == n_sources && n_models > 1;   // model i belongs to source i
+  // the copy streams start after what `stream` has been given so far (the parameters above; earlier calls that use
+  // the staging area)
+  TWK_CUDA(cudaEventRecord(ctx->ev_first, stream));
+  TWK_CUDA(cudaStreamWaitEvent(ctx->copy_in, ctx->ev_first, 0));
+  TWK_CUDA(cudaStreamWaitEvent(ctx->copy_out, ctx->ev_first, 0));
+  for (int c = 0; c < n_chunks; ++c) {
+    const size_t off = bound[c], m = bound[c + 1] - off;
+    if (model_id) TWK_CUDA(cudaMemcpyAsync(d_mid + off, model_id + off, m * 4, cudaMemcpyHostToDevice, ctx->copy_in));
+    TWK_CUDA(cudaMemcpyAsync(d_zeta + 2 * off, zeta + 2 * off, m * 16, cudaMemcpyHostToDevice, ctx->copy_in));
+    TWK_CUDA(cudaEventRecord(ctx->ev_in[c], ctx->copy_in));
+  }
+  int launches = 0;
+  for (int c = 0; c < n_chunks; ++c) {
+    const size_t off = bound[c], m = bound[c + 1] - off;
+    const size_t po = identity ? off : 0;
+    TWK_CUDA(cudaStreamWaitEvent(stream, ctx->ev_in[c], 0));
+    const int r2 = twk_magnify(ctx, identity ? m : n_models, d_s + po, d_q + po, d_rho + po, m, model_id ? d_mid + off : nullptr,
+                               d_zeta + 2 * off, rel_tol, d_mu + off, out_err ? d_err + off : nullptr,
+                               out_nsamples ? d_ns + off : nullptr, out_status ? d_st + off : nullptr, stream_);
+    if (r2 != TWK_OK) {
+      cudaStreamSynchronize(ctx->copy_in);
+      cudaStreamSynchronize(ctx->copy_out);
+      cudaStreamSynchronize(stream);
+      return r2;
+    }
+    launches += ctx->last_launches;
+    TWK_CUDA(cudaEventRecord(ctx->ev_done[c], stream));
+    TWK_CUDA(cudaStreamWaitEvent(ctx->copy_out, ctx->ev_done[c], 0));
+    TWK_CUDA(cudaMemcpyAsync(out_mu + off, d_mu + off, m * 8, cudaMemcpyDeviceToHost, ctx->copy_out));
+    if (out_err) TWK_CUDA(cudaMemcpyAsync(out_err + off, d_err + off, m * 8, cudaMemcpyDeviceToHost, ctx->copy_out));
+    if (out_nsamples) TWK_CUDA(cudaMemcpyAsync(out_nsamples + off, d_ns + off, m * 4, cudaMemcpyDeviceToHost, ctx->copy_out));
+    if (out_status) TWK_CUDA(cudaMemcpyAsync(out_status + off, d_st + off, m * 4, cudaMemcpyDeviceToHost, ctx->copy_out));
+  }
+  ctx->last_launches = launches;
+  TWK_CUDA(cudaEventRecord(ctx->ev_last, ctx->copy_out));
+  TWK_CUDA(cudaStreamWaitEvent(stream, ctx->ev_last, 0));   // `stream` stays the one order of everything this call did
   TWK_CUDA(cudaStreamSynchronize(stream));
   return TWK_OK;
 }
@@ -710,6 +801,9 @@ int static_context(twk_ctx** out) {
     c.ws = static_cast<char*>(base);
     c.stage = nullptr;
     c.stage_bytes = 0;
+    c.copy_in = c.copy_out = nullptr;
+    c.ev_first = c.ev_last = nullptr;
+    for (int i = 0; i < kHostChunksMax; ++i) c.ev_in[i] = c.ev_done[i] = nullptr;
     c.last_launches = 0;
     c.timing = 0;
     c.ev_used = 0;

@@ -610,3 +610,34 @@ def test_host_buffer_entry_point(ctx):
     assert np.array_equal(out["mu"], g["mu"]) and np.array_equal(out["nsamples"], g["nsamples"])
     st = ctx.twk_last_stats()
     assert st["n_launches"] >= 1
+
+
+def test_host_buffer_entry_point_in_chunks():
+    """A batch of more than 2,097,152 sources passes twk_magnify_host in chunks whose copies overlap the kernels of the
+    neighbouring chunk (include/twk.h): per-source results are those of ONE twk_magnify call on the whole batch, bit for
+    bit, with a model_id array (config 3: 2,300 models x 1,000 epochs, a ragged last chunk), with NULL ids and one model
+    per source (the per-chunk parameter offset), with NULL ids and a single model, from pageable and from pinned buffers."""
+    import torch
+    import paper_2501_03322_b200 as P
+    c = P.Context(2_300_000)
+    rng = np.random.default_rng(250103340)
+    wl3 = W.config3(n_models=2300)
+    n = 2_250_001
+    lu = lambda a, b, k: np.exp(rng.uniform(np.log(a), np.log(b), k))
+    per_source = W.Workload("one model per source", lu(0.3, 3, n), lu(1e-5, 1, n), lu(1e-4, 1e-2, n),
+                            np.arange(n, dtype=np.int32), np.ascontiguousarray(rng.uniform(-1, 1, (n, 2))), 1e-3)
+    single = W.Workload("one model", np.array([1.0]), np.array([0.1]), np.array([1e-2]), np.zeros(n, np.int32),
+                        np.ascontiguousarray(rng.uniform(-1.5, 1.5, (n, 2))), 1e-3)
+    for wl, tol, ids in ((wl3, 1e-4, True), (per_source, 1e-3, False), (single, 1e-3, False)):
+        g = c.magnify_workload(wl, tol)                     # device buffers, one call
+        out = c.twk_magnify_host(wl.s, wl.q, wl.rho, wl.zeta, wl.model_id if ids else None, tol)
+        assert c.twk_last_stats()["n_launches"] >= 8, "the batch did not go through in chunks"
+        for key in ("mu", "err"):
+            assert np.array_equal(out[key], g[key], equal_nan=True), (wl.name, key)
+        assert np.array_equal(out["nsamples"], g["nsamples"]) and np.array_equal(out["status"], g["status"].astype(np.uint32))
+    # pinned host buffers, only mu asked for
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    out = dict(mu=torch.empty(wl3.n_sources, dtype=torch.float64).pin_memory())
+    c.twk_magnify_host(pin(wl3.s), pin(wl3.q), pin(wl3.rho), pin(wl3.zeta), pin(wl3.model_id), 1e-4, out=out)
+    assert np.array_equal(out["mu"].numpy(), c.magnify_workload(wl3, 1e-4)["mu"])
+    c.close()
