@@ -641,3 +641,21 @@ def test_host_buffer_entry_point_in_chunks():
     c.twk_magnify_host(pin(wl3.s), pin(wl3.q), pin(wl3.rho), pin(wl3.zeta), pin(wl3.model_id), 1e-4, out=out)
     assert np.array_equal(out["mu"].numpy(), c.magnify_workload(wl3, 1e-4)["mu"])
     c.close()
+
+
+def test_source_order_and_batch_size_do_not_change_a_source(ctx):
+    """Stage 1 hands a batch of a few waves to its CTAs in groups whose sources are spread evenly over the batch (column c
+    of group g = source g + c * n_groups), a large batch in groups of consecutive sources (csrc/twk_api.cu launch_stage1).
+    A source's result must not depend on which path took it, on its position in the batch or on its neighbours: the same
+    sources alone (strided groups, ragged: columns without a source), shuffled, and inside a batch of 500,000 (contiguous
+    groups) give the same bits."""
+    big = W.config3(n_models=500)                                   # 500,000 sources: contiguous groups
+    gb = ctx.magnify_workload(big, 1e-4)
+    assert ctx.twk_last_stats()["n_stage2"] > 10000
+    rng = np.random.default_rng(250103341)
+    for k in (5, 10_007, 57_001):
+        idx = np.sort(rng.choice(big.n_sources, k, replace=False))
+        for order in (idx, rng.permutation(idx)):
+            g = ctx.magnify_workload(big.subset(order), 1e-4)
+            for key in ("mu", "err", "nsamples", "status"):
+                assert np.array_equal(g[key], gb[key][order]), (k, key)
