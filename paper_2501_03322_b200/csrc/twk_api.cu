@@ -122,22 +122,33 @@ void launch_stage1(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t
   a.n_big = groups;
   a.tail_group = (int)group;
   a.interleave = 0;
+  a.il_shift = 0;
   if (group == twk::kS1Group && groups > 8 * resident) {
     a.n_big = groups - 2 * resident;
     a.tail_group = 16;
     groups = a.n_big + (n_sources - a.n_big * group + 15) / 16;
   } else {
-    // a batch of a few waves at most: the sources of a group are spread evenly over the batch (column c of group g is
-    // source g + c * groups), so that a run of expensive neighbours is shared by many CTAs.  Measured (stage 1,
-    // contiguous groups -> these): config 2 0.256 -> 0.09 ms, Fig.5 resonant map 1.67 -> 1.4 ms, 64 light curves of
-    // config 3 0.71 -> 0.45 ms; a batch of many waves (config 4) does not care and keeps its contiguous groups (and
-    // their coalesced seed rows).
+    // a batch of a few waves at most: a group is made of blocks of consecutive sources spread evenly over the batch (block b
+    // of group g starts at source (g + b * groups) * B), so that a run of expensive neighbours is shared by many CTAs.
+    // B = 4 (one full 32-byte sector per seed row and block) for groups of 16 sources or more, single sources below.
+    // Measured (stage 1, contiguous groups -> these): config 2 0.256 -> 0.09 ms, Fig.5 resonant map 1.67 -> 1.42 ms, 64
+    // light curves of config 3 0.71 -> 0.5 ms; a batch of many waves (config 4) does not care and keeps its contiguous
+    // groups (and their coalesced seed rows).
+    a.il_shift = group >= 16 ? 2 : 0;
+    const long long B = 1ll << a.il_shift;
+    group = (group + B - 1) / B * B;
+    const long long blocks = (n_sources + B - 1) / B, per_group = group / B;
+    groups = (blocks + per_group - 1) / per_group;
+    a.group = (int)group;
+    a.tail_group = (int)group;
     a.n_big = groups;
     a.interleave = 1;
   }
   const int grid = (int)(groups < resident ? groups : resident);
-  if (a.guard) twk::stage1_kernel<true><<<grid, twk::kThreads, smem, stream>>>(a);
-  else twk::stage1_kernel<false><<<grid, twk::kThreads, smem, stream>>>(a);
+  if (a.guard && a.interleave) twk::stage1_kernel<true, true><<<grid, twk::kThreads, smem, stream>>>(a);
+  else if (a.guard) twk::stage1_kernel<true, false><<<grid, twk::kThreads, smem, stream>>>(a);
+  else if (a.interleave) twk::stage1_kernel<false, true><<<grid, twk::kThreads, smem, stream>>>(a);
+  else twk::stage1_kernel<false, false><<<grid, twk::kThreads, smem, stream>>>(a);
 }
 
 constexpr int kHostChunksMax = 8;

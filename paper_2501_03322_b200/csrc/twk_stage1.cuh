@@ -49,10 +49,11 @@ struct Stage1Args {
   int group;             // sources per group, 1..64 (smaller for small batches: more CTAs get work)
   long long n_big;       // the first n_big groups have `group` sources, the rest of the batch goes out in groups of
   int tail_group;        // `tail_group` sources: the last wave of a large batch ends together
-  int interleave;        // 1 (batches of a few waves at most): column c of group g is source g + c * n_big (n_big = the number
-                         // of groups) instead of g * group + c: neighbouring sources -- the epochs of a light curve around
-                         // its peak, the pixels of a map along a caustic -- are equally expensive, and with one or two
-                         // groups per CTA the slowest CTA is the launch
+  int interleave;        // 1 (batches of a few waves at most): a group is made of blocks of 2^il_shift consecutive sources,
+  int il_shift;          // the blocks n_big (= the number of groups) apart, instead of `group` consecutive sources:
+                         // neighbouring sources -- the epochs of a light curve around its peak, the pixels of a map along
+                         // a caustic -- are equally expensive, and with one or two groups per CTA the slowest CTA is the
+                         // launch
   int final_stage;       // 1: there is no refinement stage (max_samples < 128): cap status instead of pending
   const double* seeds;   // [kSeedDoubles][n_sources] seed blocks written by stage 0
   int* cursor;           // group fetch counter (zeroed before launch)
@@ -80,7 +81,9 @@ __host__ __device__ constexpr size_t stage1_smem_bytes() {
 
 // kGuard: the L-4 hidden-crossing term (twk_options.hidden_crossing_guard) is compiled into its own instance of the
 // kernel: the default instance carries no trace of it (the loop is sensitive to every extra instruction)
-template <bool kGuard>
+// kSpread: the groups of a batch of a few waves (Stage1Args::interleave), likewise an instance of its own: the instance
+// that takes the large batches is the contiguous-group kernel and nothing else
+template <bool kGuard, bool kSpread>
 __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Args p) {
   extern __shared__ double sm[];
   double* recs = sm;                                          // [26][64] records of the current source
@@ -102,7 +105,7 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
   const RecRef mine{recs + t, kThreads};
   const RecRef next{recs + ((t + 1) & (kThreads - 1)), kThreads};
   const long long n = p.b.n_sources;
-  const bool il = p.interleave != 0;
+  constexpr bool il = kSpread;
   const long long n_big = p.n_big, n_in_big = n_big * p.group;
   const long long n_groups = il ? n_big : n_big + (n - n_in_big + p.tail_group - 1) / p.tail_group;
   int parity = 0;
@@ -116,12 +119,16 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
     const int G = (il || g < n_big) ? p.group : p.tail_group;
     const long long base = (g < n_big) ? g * p.group : n_in_big + (g - n_big) * p.tail_group;   // first source of the group
     // source of column `col` of the group (phase 2 reads it from res_src)
-    auto src_at = [&](int col) -> long long { return il ? g + (long long)col * n_groups : base + col; };
+    auto src_at = [&](int col) -> long long {
+      return il ? ((g + (long long)(col >> p.il_shift) * n_groups) << p.il_shift) + (col & ((1 << p.il_shift) - 1)) : base + col;
+    };
     // ---- phase 1: parameters and centre roots of source base + t --------------------------------------------------
     {
       const long long src = src_at(t);
-      if (t < G) res_src[t] = (int)src;
-      if (t < G && src >= n) prm[7 * kS1Group + t] = code_as_double(0);   // no source in this column (phase 2 skips it)
+      if (il && t < G) {
+        res_src[t] = (int)src;
+        if (src >= n) prm[7 * kS1Group + t] = code_as_double(0);   // no source in this column (phase 2 skips it)
+      }
       if (t < G && src < n) {
         const SourceParams S = load_source(p.b, src);
         prm[0 * kS1Group + t] = S.L.s;
@@ -234,7 +241,7 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
         __syncthreads();
       }
       if (p.dump) {
-        double* d = p.dump + (size_t)res_src[i] * (kRecDoubles * kThreads);
+        double* d = p.dump + (size_t)(il ? (long long)res_src[i] : base + i) * (kRecDoubles * kThreads);
 #pragma unroll 1
         for (int e = 0; e < kRecDoubles; ++e) d[e * kThreads + t] = mine.at(e);
       }
@@ -262,7 +269,7 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
         if (t == 0) {
           const double S2 = sq[0] + sq[1], E2 = E * E, den = E2 + 64.0 * S2;
           const bool spread = E * E2 * E2 > 1.5 * p.tol * fabs(A) * den * den;   // E / (1 + 64 S2 / E^2)^2 > 1.5 tol |A|
-          p.list[slot] = (int32_t)res_src[i] | (spread ? (int32_t)0x80000000 : 0);
+          p.list[slot] = (int32_t)(il ? (long long)res_src[i] : base + i) | (spread ? (int32_t)0x80000000 : 0);
         }
         if (slot < p.handoff_slots) {
           double* h = p.handoff + (size_t)slot * kHandDoubles;
@@ -273,7 +280,7 @@ __global__ void __launch_bounds__(kThreads, kS1CtasPerSM) stage1_kernel(Stage1Ar
           if (t < kSeedDoubles) h[(kRecDoubles + 2) * kThreads + t] = seeds[t * kS1Group + i];
           if (t >= 32 && t < 32 + 9) {   // header: what stage 2 needs to start this source without looking anything up
             const int k = t - 32;
-            h[kHandHeader + k] = (k == 0) ? __longlong_as_double((long long)res_src[i])
+            h[kHandHeader + k] = (k == 0) ? __longlong_as_double(il ? (long long)res_src[i] : base + i)
                                           : (k == 8) ? code_as_double(code & 255) : prm[(k - 1) * kS1Group + i];
           }
         }
