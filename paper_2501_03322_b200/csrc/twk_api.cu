@@ -113,8 +113,20 @@ void launch_stage1(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t
   static_assert(twk::stage1_smem_bytes() <= 48 * 1024, "stage-1 shared memory needs the opt-in attribute");
   // groups of up to 64 sources per CTA pass; a small batch takes smaller groups so that every resident CTA gets work
   const long long resident = (long long)sms * twk::kS1CtasPerSM;
-  long long group = (n_sources + resident - 1) / resident;
-  group = group < 4 ? 4 : (group > twk::kS1Group ? twk::kS1Group : group);
+  // group size: about 8 groups per resident CTA, so that the cursor can even out what the groups cost (a group of 64 is
+  // 0.3 ms of one CTA, and a batch of two waves used to end with half of the CTAs waiting for the other half), but not
+  // below 16 sources (per-group set-up: a DRAM round trip and three barriers) unless the batch is too small to give every
+  // CTA 16.  Measured (stage 1, one group per CTA up to 64 -> this): 113,664 config-3 sources 0.78 -> 0.68 ms, Fig.5
+  // resonant map 1.42 -> 1.31 ms, config 5 0.89 -> 0.78 ms, 400,000 sources 2.36 -> 2.29 ms; 4 groups per CTA gain a little
+  // less, 2 nothing.
+  long long group = (n_sources + 8 * resident - 1) / (8 * resident);
+  {
+    const long long g1 = (n_sources + resident - 1) / resident;   // one group per CTA
+    long long lo = g1 < 16 ? g1 : 16;
+    if (lo < 4) lo = 4;
+    if (group < lo) group = lo;
+  }
+  group = group > twk::kS1Group ? twk::kS1Group : group;
   a.group = (int)group;
   long long groups = (n_sources + group - 1) / group;
   // a large batch ends in small groups: its last two waves of 64-source groups go out as groups of 16, so that the
