@@ -394,8 +394,25 @@ def main():
     ps_maxdev = float(((out_ps["out_mu"] / out["out_mu"]) - 1).abs().max().item())
     ctx_ps.close()
     ctx.close()
+    # ---- for information: the same batch with the hidden-crossing guard (reading L-4, an extension of Eq.(17)) ----
+    ctx_hg = P.Context(n, hidden_crossing_guard=1)
+    out_hg = {k: torch.empty_like(v) for k, v in out.items()}
+    for _ in range(2):
+        ctx_hg.twk_magnify(d["s"], d["q"], d["rho"], d["zeta"], d["model_id"], wl.rel_tol, **out_hg)
+    barrier()
+    h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    h0.record()
+    for _ in range(args.steps):
+        ctx_hg.twk_magnify(d["s"], d["q"], d["rho"], d["zeta"], d["model_id"], wl.rel_tol, **out_hg)
+    h1.record()
+    barrier()
+    ms_hg = h0.elapsed_time(h1)
+    hg_dev = ((out_hg["out_mu"] / out["out_mu"]) - 1).abs()
+    hg_changed = int((hg_dev > wl.rel_tol).sum().item())
+    hg_maxdev = float(hg_dev.max().item())
+    ctx_hg.close()
 
-    ms, ms_e2e, ms_ps = max_over_ranks([ms, ms_e2e, ms_ps], dev, world)
+    ms, ms_e2e, ms_ps, ms_hg = max_over_ranks([ms, ms_e2e, ms_ps, ms_hg], dev, world)
 
     if rank == 0:
         peaks = {}
@@ -448,6 +465,12 @@ def main():
                                        "max_rel_dev_from_contour": ps_maxdev,
                                        "note": "option point_source_test=1 (SURVEY N1, P:122): sources passing the "
                                                "quadrupole and ghost-image tests skip the contour; NOT the headline"},
+            "with_hidden_crossing_guard": {"value": world * n * args.steps / (ms_hg * 1e-3), "unit": UNIT,
+                                           "ms_per_step": ms_hg / args.steps, "sources_changed_beyond_tol": hg_changed,
+                                           "max_rel_change": hg_maxdev,
+                                           "note": "option hidden_crossing_guard=1 (DESIGN.md reading L-4: an extension of "
+                                                   "Eq.(17) that closes the hidden double crossings the paper's estimate "
+                                                   "cannot see; no stage 1.5 with it); NOT the headline"},
             "gpu_launches": R["launches"] * args.steps,
             "clocks": clocks,
             "roofline": {"bound": "alu", "kernel": "stage1_kernel (64 seeded point solves + 64 intervals per source)",
