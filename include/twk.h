@@ -84,7 +84,9 @@ typedef struct {
                         /* Eq.(17) (reading L-4), default 0.  A source boundary that dips into a caustic and  */
                         /* out again between two adjacent samples is invisible to Eq.(17); the ghost pair's separation  */
                         /* at the two samples and their neighbours predicts it, and the area it would hide is added to   */
-                        /* the interval's estimate.  Changes ~1 source in 50,000 (those it is for), costs nothing else.  */
+                        /* the interval's estimate.  Changes ~1 source in 50,000 (those it is for) and no other result;   */
+                        /* the kernels with the guard are separate instances and slower (config 3 of the bench: 107 M   */
+                        /* instead of 147 M magnifications/s on a B200).                                                */
   int frame;            /* frame of the zeta passed in: 0 = centre of mass (the paper's, Eq.(2)); 1 = primary lens at   */
                         /* the origin (z1 = -q s/(1+q) is added to every zeta; BASELINE configs 1 and 2 are stated so)  */
 } twk_options;

@@ -111,7 +111,6 @@ void launch_stage1(int sms, long long n_sources, twk::Stage1Args a, cudaStream_t
   }
   const size_t smem = twk::stage1_smem_bytes();   // below the 48 KB default limit: no opt-in needed
   static_assert(twk::stage1_smem_bytes() <= 48 * 1024, "stage-1 shared memory needs the opt-in attribute");
-  // groups of up to 64 sources per CTA pass; a small batch takes smaller groups so that every resident CTA gets work
   const long long resident = (long long)sms * twk::kS1CtasPerSM;
   // group size: about 8 groups per resident CTA, so that the cursor can even out what the groups cost (a group of 64 is
   // 0.3 ms of one CTA, and a batch of two waves used to end with half of the CTAs waiting for the other half), but not

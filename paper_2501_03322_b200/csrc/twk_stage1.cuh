@@ -1,6 +1,7 @@
 // twk_stage1.cuh -- stage 1 of twk_magnify: the first iteration (64 uniform boundary samples) of EVERY source.
 //
-// One 64-thread CTA takes a group of up to 64 consecutive sources from an atomic cursor:
+// One 64-thread CTA takes a group of up to 64 sources from an atomic cursor (consecutive sources in a batch of many waves; in
+// a smaller batch blocks of 4 consecutive sources spread evenly over the batch -- the kSpread instance, see Stage1Args):
 //   phase 1  thread i loads the parameters and the seed block of source i (stage 0: the five planet-frame roots of the
 //            point source at the source's CENTRE and their first-order response to a source displacement);
 //   phase 2  for each source of the group: thread t solves boundary sample t by seeded Newton on the undeflated
